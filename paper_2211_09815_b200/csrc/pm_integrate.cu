@@ -1,0 +1,192 @@
+// pm_integrate.cu -- fused kick/drift updates of the reversible KDK integrator, objective residual.
+//
+// PAPER.md eq. 16 (L172): K: p += acc K;  D: x += p D;  eq. 49 (L393): the adjoint step undoes them in
+// reverse order with the time arguments swapped, D(tc,ta,tb) = -D(tc,tb,ta) (L389), and advances
+// xi -= alpha K, pi -= xi D alongside.  The state is held in fixed point (s: int32 * 2^-fbits cells,
+// p: int64 * 2^-PBITS) so that "+= round(v)" followed by "+= round(-v)" restores it bit for bit: the
+// reverse pass then re-evaluates F at exactly the forward positions (
+// L371 names "more precise floating-point numbers" as the paper's remedy for fp32 irreversibility).
+#include "pm_internal.cuh"
+
+namespace pm {
+
+static inline int ew_blocks(long long n)
+{
+    long long b = (n + 255) / 256;
+    if (b > 148 * 16) b = 148 * 16;
+    if (b < 1) b = 1;
+    return (int)b;
+}
+
+__global__ void __launch_bounds__(256) state_from_float_kernel(long long n3, const float *__restrict__ s, const float *__restrict__ p,
+                                                               double sscale, double pscale, int *__restrict__ sf,
+                                                               long long *__restrict__ pf)
+{
+    long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n3; i += stride) {
+        sf[i] = (int)__double2ll_rn((double)s[i] * sscale);
+        pf[i] = __double2ll_rn((double)p[i] * pscale);
+    }
+}
+
+__global__ void __launch_bounds__(256) state_to_float_kernel(long long n3, const int *__restrict__ sf, const long long *__restrict__ pf,
+                                                             double inv_sscale, double inv_pscale, float *__restrict__ s,
+                                                             float *__restrict__ p)
+{
+    long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n3; i += stride) {
+        if (s) s[i] = (float)((double)sf[i] * inv_sscale);
+        if (p) p[i] = (float)((double)pf[i] * inv_pscale);
+    }
+}
+
+// Ks = K * 2^PBITS, Ds = D * 2^fbits / 2^PBITS.  ADJ also advances xi, pi with the plain K, D.
+template <bool ADJ>
+__global__ void __launch_bounds__(256) kick_drift_kernel(long long n3, double Ks, double Ds, float K, float D,
+                                                         int *__restrict__ s, long long *__restrict__ p,
+                                                         const float *__restrict__ acc, float *__restrict__ xi,
+                                                         float *__restrict__ pi, const float *__restrict__ alpha)
+{
+    long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n3; i += stride) {
+        long long pv = p[i];
+        if (Ks != 0.0) {
+            pv += __double2ll_rn((double)acc[i] * Ks);
+            p[i] = pv;
+        }
+        if (Ds != 0.0) {
+            unsigned int sv = (unsigned int)s[i];
+            sv += (unsigned int)(int)__double2ll_rn((double)pv * Ds);  // wraps: displacement is periodic mod 2^(32-fbits) cells
+            s[i] = (int)sv;
+        }
+        if (ADJ) {
+            float x = xi[i];
+            if (Ks != 0.0) {
+                x = fmaf(-alpha[i], K, x);
+                xi[i] = x;
+            }
+            if (Ds != 0.0) pi[i] = fmaf(-x, D, pi[i]);
+        }
+    }
+}
+
+// r = rho/nbar - 1 - target, in place in the padded mesh; J += 1/2 sum r^2 (fp64)
+__global__ void __launch_bounds__(256) objective_kernel(int Nx, int Ny, int Nz, int zs, float inv_nbar, float *__restrict__ mesh,
+                                                        const float *__restrict__ target, double *__restrict__ J)
+{
+    __shared__ double red[8];
+    long long ng = (long long)Nx * Ny * Nz;
+    long long stride = (long long)gridDim.x * blockDim.x;
+    double part = 0.0;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < ng; i += stride) {
+        int iz = (int)(i % Nz);
+        long long row = i / Nz;
+        size_t o = (size_t)row * zs + iz;
+        float r = fmaf(mesh[o], inv_nbar, -1.f) - target[i];
+        mesh[o] = r;
+        part += 0.5 * (double)r * (double)r;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = part;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+        for (int k = 0; k < 8; k++) t += red[k];
+        J[1 + blockIdx.x] = t;  // per-block partial; summed in a fixed order below (bit-reproducible J)
+    }
+}
+
+__global__ void objective_final_kernel(int nblocks, double *__restrict__ J)
+{
+    if (threadIdx.x == 0 && blockIdx.x == 0) {
+        double t = 0.0;
+        for (int k = 0; k < nblocks; k++) t += J[1 + k];
+        J[0] = t;
+    }
+}
+
+__global__ void __launch_bounds__(256) combine_kernel(long long n3, const float *__restrict__ xi, const float *__restrict__ pi,
+                                                      float ratio, float *__restrict__ out)
+{
+    long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n3; i += stride)
+        out[i] = fmaf(pi[i], ratio, xi[i]);
+}
+
+int state_from_float(pm_ctx *c, const float *s, const float *p)
+{
+    long long n3 = 3 * c->g.np;
+    Timer t(c, TC_CONVERT, 20.0 * n3);
+    state_from_float_kernel<<<ew_blocks(n3), 256, 0, c->stream>>>(n3, s, p, ldexp(1.0, c->g.fbits), ldexp(1.0, PBITS), c->s, c->p);
+    PM_LAUNCH_CHECK(c, "state_from_float_kernel");
+    t.stop();
+    return PM_OK;
+}
+
+int state_to_float(pm_ctx *c, float *s, float *p)
+{
+    long long n3 = 3 * c->g.np;
+    Timer t(c, TC_CONVERT, 20.0 * n3);
+    state_to_float_kernel<<<ew_blocks(n3), 256, 0, c->stream>>>(n3, c->s, c->p, ldexp(1.0, -c->g.fbits), ldexp(1.0, -PBITS), s, p);
+    PM_LAUNCH_CHECK(c, "state_to_float_kernel");
+    t.stop();
+    return PM_OK;
+}
+
+int kick_drift(pm_ctx *c, double K, double D)
+{
+    long long n3 = 3 * c->g.np;
+    double Ks = ldexp(K, PBITS), Ds = ldexp(D, c->g.fbits - PBITS);
+    Timer t(c, TC_KICK_DRIFT, (K != 0.0 ? 20.0 : 8.0) * n3 + (D != 0.0 ? 8.0 * n3 : 0.0));
+    kick_drift_kernel<false><<<ew_blocks(n3), 256, 0, c->stream>>>(n3, Ks, Ds, (float)K, (float)D, c->s, c->p, c->acc, nullptr,
+                                                                   nullptr, nullptr);
+    PM_LAUNCH_CHECK(c, "kick_drift_kernel");
+    t.stop();
+    if (D != 0.0) c->sorted_valid = false;
+    return PM_OK;
+}
+
+int kick_drift_adj(pm_ctx *c, double K, double D)
+{
+    long long n3 = 3 * c->g.np;
+    double Ks = ldexp(K, PBITS), Ds = ldexp(D, c->g.fbits - PBITS);
+    Timer t(c, TC_KICK_DRIFT, (K != 0.0 ? 32.0 : 12.0) * n3 + (D != 0.0 ? 16.0 * n3 : 0.0));
+    kick_drift_kernel<true><<<ew_blocks(n3), 256, 0, c->stream>>>(n3, Ks, Ds, (float)K, (float)D, c->s, c->p, c->acc, c->xi,
+                                                                  c->pi, c->alpha);
+    PM_LAUNCH_CHECK(c, "kick_drift_kernel<adj>");
+    t.stop();
+    if (D != 0.0) c->sorted_valid = false;
+    return PM_OK;
+}
+
+int objective_residual(pm_ctx *c, float *mesh, const float *target, double nbar)
+{
+    const Geometry &g = c->g;
+    Timer t(c, TC_OBJECTIVE, 12.0 * (double)g.ng);
+    int nb = ew_blocks(g.ng);  // <= 148 * 16 < the 4096 doubles of scal
+    objective_kernel<<<nb, 256, 0, c->stream>>>(g.N[0], g.N[1], g.N[2], g.zs, (float)(1.0 / nbar), mesh, target, c->scal);
+    objective_final_kernel<<<1, 32, 0, c->stream>>>(nb, c->scal);
+    c->n_own++;
+    PM_LAUNCH_CHECK(c, "objective_kernel");
+    t.stop();
+    return PM_OK;
+}
+
+int combine_dJ_ds0(pm_ctx *c, float *out)
+{
+    long long n3 = 3 * c->g.np;
+    Timer t(c, TC_CONVERT, 12.0 * n3);
+    combine_kernel<<<ew_blocks(n3), 256, 0, c->stream>>>(n3, c->xi, c->pi, (float)c->p_over_s0, out);
+    PM_LAUNCH_CHECK(c, "combine_kernel");
+    t.stop();
+    return PM_OK;
+}
+
+int fill_zero(pm_ctx *c, void *ptr, size_t bytes)
+{
+    PM_CUDA(c, cudaMemsetAsync(ptr, 0, bytes, c->stream));
+    return PM_OK;
+}
+
+}  // namespace pm

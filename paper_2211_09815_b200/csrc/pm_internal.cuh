@@ -1,0 +1,166 @@
+// pm_internal.cuh -- private declarations of libpm (CUDA, sm_100a).  Not part of the ABI.
+// Shares nothing with oracle/ (the CPU fp64 oracle is test infrastructure with its own code).
+#pragma once
+#include <cuda_runtime.h>
+#include <cufft.h>
+#include <stdint.h>
+#include <string>
+#include <vector>
+
+#include "pm.h"
+
+namespace pm {
+
+// ---- tile geometry of the cell sort -----------------------------------------------------------------
+// Particles are binned by mesh tile of TX x TY x TZ cells (z contiguous in memory: 32 cells = one
+// 128-byte row of fp32) and, inside a tile, by a 3-bit class: bit 2/1/0 set when the particle sits in
+// the LAST cell layer of the tile along x/y/z, i.e. when its CIC cloud reaches into the next tile.
+constexpr int TX = 8, TY = 8, TZ = 32;
+constexpr int NCLS = 8;
+constexpr int PBITS = 36;  // momentum fixed point: p_fix = p * 2^PBITS (int64)
+
+// ---- timing classes ---------------------------------------------------------------------------------
+enum TimingClass {
+    TC_BIN_COUNT = 0,
+    TC_BIN_SCAN,
+    TC_BIN_REORDER,
+    TC_SCATTER1,
+    TC_SCATTER3,
+    TC_GATHER3,
+    TC_GATHER_GRAD,
+    TC_GATHER_FUSED,
+    TC_KSPACE_FORCE,
+    TC_KSPACE_ADJ,
+    TC_FFT_R2C,
+    TC_FFT_C2R,
+    TC_KICK_DRIFT,
+    TC_OBJECTIVE,
+    TC_CONVERT,
+    TC_NCLASSES
+};
+extern const char *const kTimingNames[TC_NCLASSES];
+
+struct TimingRec {
+    cudaEvent_t e0, e1;
+    int cls;
+    double bytes;
+};
+
+struct Geometry {
+    int N[3];        // mesh
+    int L[3];        // lattice
+    int nt[3];       // tiles per axis
+    int fbits;       // fraction bits of the absolute fixed-point coordinate
+    int zs;          // floats per z-row of a (padded) internal mesh: Nz + 2
+    long long np;    // particles of the lattice
+    long long ng;    // Nx*Ny*Nz
+    long long mesh_stride;  // floats per internal padded mesh: Nx*Ny*(Nz+2)
+    long long nk;    // complex modes Nx*Ny*(Nz/2+1)
+    int ntiles;      // nt[0]*nt[1]*nt[2]
+    int nkeys;       // ntiles * NCLS
+    unsigned long long qstep[3];  // lattice spacing in fixed point: (N << fbits) / L
+};
+
+}  // namespace pm
+
+struct pm_ctx {
+    pm::Geometry g;
+    pm_params prm;
+    std::vector<double> a;       // n+1 scale factors
+    std::vector<double> fac;     // 3 per step: K1, D, K2 (forward)
+    double p_over_s0;            // G_D(a0)/D1(a0)
+    cudaStream_t stream;
+    cufftHandle plan_r2c1, plan_c2r1, plan_r2c3, plan_c2r3;
+    bool plans_ok;
+    // workspace carve-up (device pointers)
+    float *mesh[7];              // padded in-place R2C layout, contiguous
+    uint4 *rec;                  // sorted records {X, Y, Z, j}
+    int *offsets;                // nkeys + 1 exclusive prefix of the key histogram
+    int *cursor;                 // nkeys + 1 scratch (histogram, then running cursors)
+    int *blocksum;               // scan scratch
+    int *s;                      // [np][3] int32 displacement * 2^fbits
+    long long *p;                // [np][3] int64 momentum * 2^PBITS
+    float *acc, *xi, *pi, *alpha;  // [np][3]
+    double *scal;                // device scalars: [0] = J
+    float *ktab;                 // [3 axes][3: kt, k^2, dec][ktabn] per-axis k-space tables
+    int ktabn;
+    long long cur_np;            // particles in the current sort
+    void *fft_work;
+    size_t fft_work_bytes;
+    // integrator bookkeeping
+    int t_index;                 // state is at t_{t_index}; -1 = no state
+    bool have_adjoint;
+    bool sorted_valid;           // rec/offsets describe the current state's positions
+    // instrumentation
+    bool timing_on;
+    std::vector<pm::TimingRec> trecs;
+    std::vector<cudaEvent_t> event_pool;
+    long long n_own, n_fft;
+    std::string err;
+};
+
+namespace pm {
+
+// record the last error text and return code
+int fail(pm_ctx *c, int code, const char *what, const char *detail);
+
+#define PM_CUDA(ctx, call)                                                        \
+    do {                                                                          \
+        cudaError_t e_ = (call);                                                  \
+        if (e_ != cudaSuccess) return pm::fail(ctx, PM_ECUDA, #call, cudaGetErrorString(e_)); \
+    } while (0)
+#define PM_LAUNCH_CHECK(ctx, name)                                                \
+    do {                                                                          \
+        cudaError_t e_ = cudaGetLastError();                                      \
+        if (e_ != cudaSuccess) return pm::fail(ctx, PM_ECUDA, name, cudaGetErrorString(e_)); \
+    } while (0)
+#define PM_TRY(expr)                 \
+    do {                             \
+        int rc_ = (expr);            \
+        if (rc_ != PM_OK) return rc_; \
+    } while (0)
+
+// RAII-ish bracket: t = Timer(ctx, cls, bytes); launch...; t.stop()
+struct Timer {
+    pm_ctx *c;
+    int idx;
+    Timer(pm_ctx *ctx, int cls, double bytes);
+    void stop();
+};
+
+// ---- host growth (pm_growth.cc) ---------------------------------------------------------------------
+void growth_host(double om, double a, double out[4]);  // D1, dD1/dlna, G_D, G_K
+double drift_factor_host(double om, double ac, double aa, double ab);
+double kick_factor_host(double om, double ac, double aa, double ab);
+
+// ---- binning (pm_bin.cu) ----------------------------------------------------------------------------
+// sort np particles given as absolute float positions (x != NULL) or as the ctx state s (x == NULL)
+int bin_particles(pm_ctx *c, long long np, const float *x);
+
+// ---- CIC (pm_cic.cu): operate on the sorted records of the last bin_particles -----------------------
+// val: [np][C] in ORIGINAL particle order or NULL.  mesh: C meshes, row stride zs, mesh stride ms.
+int scatter_sorted(pm_ctx *c, const float *val, int C, float *mesh, int zs, long long ms);
+int gather_sorted(pm_ctx *c, const float *mesh, int C, int zs, long long ms, float *out);
+int gather_grad_sorted(pm_ctx *c, const float *mesh, int C, int zs, long long ms, const float *cot,
+                       float cot_scale, float *out);
+// acc_j = sum_g W f_d ; alpha_j = sum_g dW (psi + sum_d pi_d f_d); meshes: psi = mesh4[0], f = mesh4[1..3]
+int gather_fused_sorted(pm_ctx *c, const float *mesh4, int zs, long long ms, const float *pi, float *acc,
+                        float *alpha);
+
+// ---- k-space (pm_kspace.cu) -------------------------------------------------------------------------
+int kspace_force(pm_ctx *c, const float2 *rho_k, float2 *f_k /*3 meshes, stride ms/2*/, double nbar);
+int kspace_adjoint(pm_ctx *c, const float2 *Pi_k /*3 meshes*/, float2 *psi_k, double nbar);
+
+// ---- integrator elementwise kernels (pm_integrate.cu) -----------------------------------------------
+int state_from_float(pm_ctx *c, const float *s, const float *p);
+int state_to_float(pm_ctx *c, float *s, float *p);
+// p += acc*K (first), then s += p*D  (K == 0 or D == 0 skip the respective half)
+int kick_drift(pm_ctx *c, double K, double D);
+// adjoint: p += acc*K; xi -= alpha*K; then s += p*D; pi -= xi*D
+int kick_drift_adj(pm_ctx *c, double K, double D);
+// r = rho/nbar - 1 - target in place in padded mesh; J into scal[0]
+int objective_residual(pm_ctx *c, float *mesh, const float *target, double nbar);
+int combine_dJ_ds0(pm_ctx *c, float *out);
+int fill_zero(pm_ctx *c, void *ptr, size_t bytes);
+
+}  // namespace pm

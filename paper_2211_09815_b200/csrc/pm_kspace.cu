@@ -1,0 +1,109 @@
+// pm_kspace.cu -- fused k-space kernels: Poisson Green's function x spectral gradient, and its transpose.
+//
+// PAPER.md eq. 9, 11 (L117-131), H0 = 1, cell units:  -k^2 varphi(k) = 3/2 Om delta(k);  the force is
+// -i k varphi(k), "4 (1 forward and 3 inverse) FFTs in total" (L131).  With delta = rho/nbar - 1 (L79;
+// the "-1" only touches k = 0, which is zeroed) and cuFFT's unnormalised transforms:
+//     f_d(k)  = +i kt_d * G(k) * rho(k),         G(k) = 3/2 Om * dec(k) / (k^2 nbar N_g),  G(0) = 0
+//     psi(k)  = -i G(k) * sum_d kt_d * Pi_d(k)   (transpose: kernel conjugated, components summed)
+// kt_d = k_d except 0 on the Nyquist plane (R10); k^2 uses the full k also there; dec = 1 or the CIC
+// deconvolution prod_d sinc(k_d/2)^-4 (R12).  Per-axis tables (kt, k^2, dec) are built on the host in fp64.
+#include "pm_internal.cuh"
+
+namespace pm {
+
+struct KGeom {
+    int N[3];
+    int nzc;            // Nz/2 + 1
+    long long nk;       // complex elements per mesh
+    long long cstride;  // complex elements between components (padded mesh stride / 2)
+    const float *tab;   // [3 axes][3: kt, k2, dec][tabn]
+    int tabn;
+    float c0;           // 3/2 Om / (nbar N_g)
+};
+
+__device__ __forceinline__ void k_factors(const KGeom &g, long long idx, float kt[3], float *G)
+{
+    int iz = (int)(idx % g.nzc);
+    long long row = idx / g.nzc;
+    int iy = (int)(row % g.N[1]);
+    int ix = (int)(row / g.N[1]);
+    const float *tx = g.tab, *ty = g.tab + 3 * g.tabn, *tz = g.tab + 6 * g.tabn;
+    kt[0] = tx[ix];
+    kt[1] = ty[iy];
+    kt[2] = tz[iz];
+    float k2 = tx[g.tabn + ix] + ty[g.tabn + iy] + tz[g.tabn + iz];
+    float dec = tx[2 * g.tabn + ix] * ty[2 * g.tabn + iy] * tz[2 * g.tabn + iz];
+    *G = (ix | iy | iz) == 0 ? 0.f : g.c0 * dec / k2;
+}
+
+__global__ void __launch_bounds__(256) kspace_force_kernel(KGeom g, const float2 *__restrict__ rho_k, float2 *__restrict__ f_k)
+{
+    long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < g.nk; idx += stride) {
+        float kt[3], G;
+        k_factors(g, idx, kt, &G);
+        float2 r = rho_k[idx];
+#pragma unroll
+        for (int d = 0; d < 3; d++) {
+            float c = kt[d] * G;  // times +i: (re, im) -> (-c im, c re)
+            f_k[(size_t)d * g.cstride + idx] = make_float2(-c * r.y, c * r.x);
+        }
+    }
+}
+
+__global__ void __launch_bounds__(256) kspace_adjoint_kernel(KGeom g, const float2 *__restrict__ Pi_k, float2 *__restrict__ psi_k)
+{
+    long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < g.nk; idx += stride) {
+        float kt[3], G;
+        k_factors(g, idx, kt, &G);
+        float re = 0.f, im = 0.f;
+#pragma unroll
+        for (int d = 0; d < 3; d++) {
+            float2 v = Pi_k[(size_t)d * g.cstride + idx];
+            re += kt[d] * v.x;
+            im += kt[d] * v.y;
+        }
+        // times -i G: (re, im) -> (G im, -G re)
+        psi_k[idx] = make_float2(G * im, -G * re);
+    }
+}
+
+static KGeom make_kgeom(pm_ctx *c, double nbar)
+{
+    KGeom k;
+    for (int d = 0; d < 3; d++) k.N[d] = c->g.N[d];
+    k.nzc = c->g.N[2] / 2 + 1;
+    k.nk = c->g.nk;
+    k.cstride = c->g.mesh_stride / 2;
+    k.tab = c->ktab;
+    k.tabn = c->ktabn;
+    k.c0 = (float)(1.5 * c->prm.omega_m / (nbar * (double)c->g.ng));
+    return k;
+}
+
+int kspace_force(pm_ctx *c, const float2 *rho_k, float2 *f_k, double nbar)
+{
+    KGeom k = make_kgeom(c, nbar);
+    int blocks = (int)((k.nk + 255) / 256);
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    Timer t(c, TC_KSPACE_FORCE, 32.0 * (double)k.nk);
+    kspace_force_kernel<<<blocks, 256, 0, c->stream>>>(k, rho_k, f_k);
+    PM_LAUNCH_CHECK(c, "kspace_force_kernel");
+    t.stop();
+    return PM_OK;
+}
+
+int kspace_adjoint(pm_ctx *c, const float2 *Pi_k, float2 *psi_k, double nbar)
+{
+    KGeom k = make_kgeom(c, nbar);
+    int blocks = (int)((k.nk + 255) / 256);
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    Timer t(c, TC_KSPACE_ADJ, 32.0 * (double)k.nk);
+    kspace_adjoint_kernel<<<blocks, 256, 0, c->stream>>>(k, Pi_k, psi_k);
+    PM_LAUNCH_CHECK(c, "kspace_adjoint_kernel");
+    t.stop();
+    return PM_OK;
+}
+
+}  // namespace pm

@@ -1,0 +1,236 @@
+"""GPU parity tests: the CUDA path (through the C ABI, via the thin binding) against the CPU fp64 oracle,
+element by element on the same seeded fp32 inputs.  Run on the B200 box with `-m gpu`.
+
+Tolerances (BASELINE.json north_star):
+  density mesh (pm_scatter vs oracle scatter of the SAME fp32 positions)  rel L2 <= 1e-5
+  final positions                                                         rms  <= 1e-4 cell
+  adjoint gradient dJ/ds0                                                 rel L2 <= 1e-3
+Kernel-level gathers / forces are fp32 against fp64: rel L2 <= 1e-5 is asserted (measured ~1e-6).
+"""
+import numpy as np
+import pytest
+
+from paper_2211_09815_b200 import inputs
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+
+def rel_l2(a, b):
+    a = np.asarray(a, dtype=np.float64)
+    b = np.asarray(b, dtype=np.float64)
+    return float(np.sqrt(np.sum((a - b) ** 2) / max(np.sum(b ** 2), 1e-300)))
+
+
+@pytest.fixture(scope="module")
+def pmlib():
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device (there is no CPU fallback)")
+    from paper_2211_09815_b200 import binding
+    return binding
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda()
+
+
+def rand_positions(rng, n, mesh, spread=1.0):
+    """positions partly outside [0, N) to exercise the periodic wrap"""
+    mesh = np.asarray(mesh, dtype=np.float64)
+    x = (rng.random((n, 3)) * (1.0 + 2 * spread) - spread) * mesh
+    return x.astype(np.float32)
+
+
+MESHES = [
+    ((8, 8, 8), (4, 4, 4)),          # a single tile in every direction (the tile is its own neighbour)
+    ((16, 16, 64), (8, 8, 32)),      # exactly 2 x 2 x 2 tiles
+    ((24, 20, 36), (12, 10, 18)),    # ragged tiles, non-power-of-two mesh
+    ((64, 64, 64), (32, 32, 32)),    # configs[0] mesh
+    ((40, 72, 96), (20, 36, 48)),    # several tiles + ragged tail on every axis
+]
+
+
+@pytest.mark.parametrize("mesh,lattice", MESHES)
+def test_scatter_gather_parity(pmlib, orc, mesh, lattice):
+    rng = np.random.default_rng(11)
+    pm = pmlib.PM(mesh, lattice, 1.0, [0.5, 1.0])
+    n = pm.np
+    x = rand_positions(rng, n, mesh)
+    # a dense clump: many particles in one cell (contention, large per-tile sums)
+    x[: n // 4] = (np.asarray(mesh) * 0.37 + rng.normal(0, 0.4, (n // 4, 3))).astype(np.float32)
+    xd = dev(x)
+    # --- scatter, unit mass (eq. 10)
+    rho = pm.scatter(xd).cpu().numpy()
+    rho_o = orc.scatter(mesh, x)
+    assert rel_l2(rho, rho_o) <= 1e-5
+    assert abs(rho.astype(np.float64).sum() - n) <= 1e-5 * n          # P1 mass conservation
+    # --- scatter with values, C = 3 and C = 1
+    val = rng.standard_normal((n, 3)).astype(np.float32) * np.exp(rng.normal(0, 2, (n, 1))).astype(np.float32)
+    m3 = pm.scatter(xd, dev(val)).cpu().numpy()
+    m3_o = orc.scatter(mesh, x, val)
+    assert rel_l2(m3, m3_o) <= 1e-5
+    m1 = pm.scatter(xd, dev(val[:, :1].copy())).cpu().numpy()
+    assert rel_l2(m1[0], m3_o[0]) <= 1e-5
+    # --- gather C = 3, C = 1
+    f = rng.standard_normal((3,) + tuple(mesh)).astype(np.float32)
+    fd = dev(f)
+    g3 = pm.gather(xd, fd).cpu().numpy()
+    g3_o = orc.gather(mesh, x, f)
+    assert rel_l2(g3, g3_o) <= 1e-5
+    g1 = pm.gather(xd, fd[0].contiguous()).cpu().numpy()
+    assert rel_l2(g1[:, 0], g3_o[:, 0]) <= 1e-5
+    # --- weight-gradient gather: scalar mesh without cotangent, 3 meshes with cotangents
+    gg = pm.gather_grad(xd, fd[0].contiguous()).cpu().numpy()
+    gg_o = orc.gather_grad(mesh, x, f[0])
+    assert rel_l2(gg, gg_o) <= 1e-5
+    cot = rng.standard_normal((n, 3)).astype(np.float32)
+    gg3 = pm.gather_grad(xd, fd, dev(cot)).cpu().numpy()
+    gg3_o = orc.gather_grad(mesh, x, f, cot)
+    assert rel_l2(gg3, gg3_o) <= 1e-5
+    # --- transpose identity <S(x, v), f> = <v, G(x, f)> on the GPU results (P2)
+    lhs = float(np.sum(m3.astype(np.float64) * f))
+    rhs = float(np.sum(val.astype(np.float64) * g3))
+    assert abs(lhs - rhs) <= 1e-4 * max(abs(lhs), np.sqrt(np.sum(val.astype(np.float64) ** 2) * np.sum(g3.astype(np.float64) ** 2)) * 1e-2)
+    pm.close()
+
+
+def test_scatter_is_bit_reproducible_and_order_independent(pmlib):
+    mesh, lattice = (48, 40, 64), (24, 20, 32)
+    rng = np.random.default_rng(5)
+    pm = pmlib.PM(mesh, lattice, 1.0, [0.5, 1.0])
+    x = rand_positions(rng, pm.np, mesh, spread=0.0)
+    a = pm.scatter(dev(x)).cpu().numpy()
+    b = pm.scatter(dev(x)).cpu().numpy()
+    c = pm.scatter(dev(x[rng.permutation(pm.np)])).cpu().numpy()
+    assert np.array_equal(a, b)
+    assert np.array_equal(a, c)
+    pm.close()
+
+
+def test_edge_cases(pmlib, orc):
+    mesh, lattice = (16, 16, 32), (8, 8, 16)
+    pm = pmlib.PM(mesh, lattice, 1.0, [0.5, 1.0])
+    # empty input: mesh of zeros
+    x0 = torch.empty((0, 3), dtype=torch.float32, device="cuda")
+    rho = pm.scatter(x0)
+    assert float(rho.abs().max()) == 0.0
+    # fewer particles than the lattice holds; exact integers and the upper box edge
+    x = np.array([[0, 0, 0], [15.999999, 15.999999, 31.999998], [16.0, 16.0, 32.0], [-0.25, 3.5, 7.75],
+                  [1e-9, 5, 5], [-1e-9, 5, 5]], dtype=np.float32)
+    rho = pm.scatter(dev(x)).cpu().numpy()
+    assert rel_l2(rho, orc.scatter(mesh, x)) <= 1e-6
+    f = np.random.default_rng(2).standard_normal((3,) + mesh).astype(np.float32)
+    assert rel_l2(pm.gather(dev(x), dev(f)).cpu().numpy(), orc.gather(mesh, x, f)) <= 1e-5
+    # argument errors: wrong C, too many particles
+    with pytest.raises(pmlib.PMError):
+        pm.scatter(torch.zeros((pm.np + 1, 3), dtype=torch.float32, device="cuda"))
+    with pytest.raises(pmlib.PMError):
+        pm.gather(dev(x), dev(f[:2]))
+    # out-of-order integrator calls
+    with pytest.raises(pmlib.PMError) as e:
+        pm.step_fwd(1)
+    assert e.value.code == pmlib.PM_ESTATE
+    pm.close()
+    with pytest.raises(pmlib.PMError):
+        pmlib.PM((16, 16, 31), (8, 8, 8), 1.0, [0.5, 1.0])       # odd Nz
+    with pytest.raises(pmlib.PMError):
+        pmlib.PM((16, 16, 32), (8, 8, 16), 1.0, [0.5, 0.4])      # non-monotone a
+
+
+@pytest.mark.parametrize("omega_m", [1.0, 0.3])
+def test_host_factors_match_oracle_growth(pmlib, orc, omega_m):
+    a = inputs.a_schedule(1.0 / 64, 63)
+    pm = pmlib.PM((16, 16, 16), (8, 8, 8), omega_m, a)
+    for i in (1, 2, 31, 63):
+        ah = 0.5 * (a[i - 1] + a[i])
+        K1 = orc.kick_factor(omega_m, a[i - 1], a[i - 1], ah)
+        D = orc.drift_factor(omega_m, ah, a[i - 1], a[i])
+        K2 = orc.kick_factor(omega_m, a[i], ah, a[i])
+        np.testing.assert_allclose(pm.step_factors(i), [K1, D, K2], rtol=2e-8)
+    g = pmlib.host_growth(omega_m, 0.37)
+    go = orc.growth(omega_m, 0.37)
+    gd = orc.GD_GK(omega_m, 0.37)
+    np.testing.assert_allclose(g, [go[0], go[1], gd[0], gd[1]], rtol=2e-8)
+    pm.close()
+
+
+@pytest.mark.parametrize("mesh,lattice,deconv", [((16, 16, 16), (8, 8, 8), 0), ((64, 64, 64), (32, 32, 32), 0),
+                                                 ((24, 20, 36), (12, 10, 18), 1), ((64, 64, 64), (32, 32, 32), 1)])
+def test_force_and_vjp_parity(pmlib, orc, mesh, lattice, deconv):
+    rng = np.random.default_rng(21)
+    pm = pmlib.PM(mesh, lattice, 0.3, [0.5, 1.0], deconvolve=deconv)
+    s = rng.normal(0, 1.5, (pm.np, 3))
+    x = (orc.positions(mesh, lattice, s)).astype(np.float32)
+    pi = rng.standard_normal((pm.np, 3)).astype(np.float32)
+    acc_o = orc.force(mesh, 0.3, x, deconv=deconv)
+    alpha_o = orc.force_vjp(mesh, 0.3, x, pi, deconv=deconv)
+    acc = pm.force(dev(x)).cpu().numpy()
+    assert rel_l2(acc, acc_o) <= 1e-5
+    tot = np.abs(acc.astype(np.float64).sum(axis=0))
+    assert np.all(tot <= 1e-5 * np.abs(acc).sum(axis=0))          # P3 momentum conservation
+    acc2, alpha = pm.force_vjp(dev(x), dev(pi))
+    assert np.array_equal(acc2.cpu().numpy(), acc)                # same meshes, same weights
+    assert rel_l2(alpha.cpu().numpy(), alpha_o) <= 1e-5
+    pm.close()
+
+
+def _cfg0_inputs(orc):
+    cfg = inputs.config(0)
+    s0 = inputs.zeldovich_displacement(cfg["lattice"], cfg["mesh"], seed=1, rms=0.3)
+    ratio = orc.p_over_s(cfg["omega_m"], cfg["a"][0])
+    p0 = (s0.astype(np.float64) * ratio).astype(np.float32)
+    # target: a second seed evolved forward by the ORACLE (never by the CUDA path)
+    s0t = inputs.zeldovich_displacement(cfg["lattice"], cfg["mesh"], seed=2, rms=0.3)
+    p0t = (s0t.astype(np.float64) * ratio).astype(np.float32)
+    s_nt, _, _ = orc.run_fwd(cfg["mesh"], cfg["lattice"], cfg["omega_m"], cfg["a"], s0t, p0t)
+    xt = orc.positions(cfg["mesh"], cfg["lattice"], s_nt)
+    nbar = np.prod(cfg["lattice"]) / np.prod(cfg["mesh"])
+    target = (orc.scatter(cfg["mesh"], xt) / nbar - 1.0).astype(np.float32)
+    return cfg, s0, p0, target
+
+
+def test_config0_forward_adjoint_parity(pmlib, orc):
+    cfg, s0, p0, target = _cfg0_inputs(orc)
+    ref = orc.run_fwd_adj(cfg["mesh"], cfg["lattice"], cfg["omega_m"], cfg["a"], s0, p0, target)
+    pm = pmlib.PM(cfg["mesh"], cfg["lattice"], cfg["omega_m"], cfg["a"])
+    out = pm.run_fwd_adj(dev(s0), dev(p0), dev(target))
+    s_n = out["s_n"].cpu().numpy().astype(np.float64)
+    rms = np.sqrt(np.mean(np.sum((s_n - ref["s_n"]) ** 2, axis=1)))
+    assert rms <= 1e-4, f"final positions rms {rms} cell"
+    assert rel_l2(out["p_n"].cpu().numpy(), ref["p_n"]) <= 1e-4
+    assert abs(out["J"] - ref["J"]) <= 1e-4 * abs(ref["J"])
+    for k in ("xi0", "pi0", "dJ_ds0"):
+        e = rel_l2(out[k].cpu().numpy(), ref[k])
+        assert e <= 1e-3, f"{k} rel L2 {e}"
+    # exact reversibility: the reverse pass returns the (fixed-point quantised) initial state bit for bit
+    fb = 22
+    s_q = np.rint(s0.astype(np.float64) * 2 ** fb) / 2 ** fb
+    p_q = np.rint(p0.astype(np.float64) * 2.0 ** 36) / 2.0 ** 36
+    assert np.array_equal(out["s_rec"].cpu().numpy(), s_q.astype(np.float32))
+    assert np.array_equal(out["p_rec"].cpu().numpy(), p_q.astype(np.float32))
+    # host-buffer entry point gives the same numbers
+    host = {k: torch.empty((pm.np, 3), dtype=torch.float32).pin_memory() for k in ("s_n", "p_n", "xi0", "pi0", "dJ_ds0")}
+    Jh = pm.run_fwd_adj_host(torch.from_numpy(s0), torch.from_numpy(p0), torch.from_numpy(target), host)
+    assert Jh == out["J"]
+    for k in host:
+        assert np.array_equal(host[k].numpy(), out[k].cpu().numpy()), k
+    pm.close()
+
+
+def test_stepwise_calls_match_whole_run(pmlib, orc):
+    cfg, s0, p0, target = _cfg0_inputs(orc)
+    pm = pmlib.PM(cfg["mesh"], cfg["lattice"], cfg["omega_m"], cfg["a"])
+    whole = pm.run_fwd_adj(dev(s0), dev(p0), dev(target))
+    pm.set_state(dev(s0), dev(p0))
+    for i in range(1, pm.n_steps + 1):
+        pm.step_fwd(i)
+    s_n, p_n = pm.get_state()
+    pm.objective(dev(target))
+    J = pm.get_objective()
+    for i in range(pm.n_steps, 0, -1):
+        pm.step_adj(i)
+    xi, pi, g = pm.get_adjoint()
+    assert J == whole["J"]
+    assert torch.equal(s_n, whole["s_n"]) and torch.equal(p_n, whole["p_n"])
+    assert torch.equal(xi, whole["xi0"]) and torch.equal(pi, whole["pi0"]) and torch.equal(g, whole["dJ_ds0"])
+    pm.close()
