@@ -92,7 +92,7 @@ static int make_geometry(const pm_params *p, Geometry *g, const char **why)
     g->nt[0] = (g->N[0] + TX - 1) / TX;
     g->nt[1] = (g->N[1] + TY - 1) / TY;
     g->nt[2] = (g->N[2] + TZ - 1) / TZ;
-    g->zs = g->N[2] + 2;
+    g->zs = (g->N[2] + 2 + 3) / 4 * 4;
     g->mesh_stride = (long long)g->N[0] * g->N[1] * g->zs;
     g->nk = (long long)g->N[0] * g->N[1] * (g->N[2] / 2 + 1);
     long long ntiles = (long long)g->nt[0] * g->nt[1] * g->nt[2];
@@ -296,7 +296,9 @@ int pm_init(pm_ctx **out, const pm_params *params, void *dev_workspace, size_t b
         c->p_over_s0 = gr[2] / gr[0];
     }
     carve_workspace(c, g, dev_workspace);
+    c->tma_ok = false;
     rc = make_plans(c);
+    if (rc == PM_OK) rc = cic_init_tensor_maps(c);
     if (rc == PM_OK) rc = upload_ktab(c);
     if (rc != PM_OK) {
         g_err_noctx = c->err;

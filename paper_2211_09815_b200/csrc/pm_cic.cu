@@ -6,15 +6,19 @@
 // Cell i_d = floor(x_d), t_d = x_d - i_d in [0,1): weight (1 - t_d) at i_d, t_d at i_d + 1 (periodic),
 // derivative -1 / +1 (floor convention, right derivative; R7).
 //
-// Input: the records sorted by (tile, class) of pm_bin.cu.  One CTA per mesh tile of TX x TY x TZ cells.
+// Input: the records sorted by (tile, class) of pm_bin.cu.  One CTA per mesh tile of TX x TY x TZ cells,
+// grid = (tiles_z, tiles_y, tiles_x).
 //
 // scatter -- OUTPUT-STATIONARY: the CTA owns the mesh points of its tile, pulls the particles of its
 //   own tile plus the last-cell-layer classes of its (up to 7) low-side neighbour tiles, accumulates in
 //   shared memory with NATIVE int32 atomics (fp32 shared atomics are CAS loops on sm_100a) in fixed
-//   point with a per-tile power-of-two scale chosen from sum|v| so that it cannot overflow, and writes
-//   every mesh point exactly once with a plain coalesced store: no zero-fill pass, no global atomics,
-//   and a result that does not depend on the order in which particles arrive (bit-reproducible).
-// gather -- the CTA stages the (TX+1)(TY+1)(TZ+1) halo of each mesh in shared memory and interpolates
+//   point with a per-tile power-of-two scale chosen from sum|v| so that it cannot overflow, converts in
+//   place and writes the tile with ONE TMA tensor store (cp.async.bulk.tensor, clipped at the mesh edge):
+//   no zero-fill pass, no global atomics, every mesh point written exactly once, and a result that does
+//   not depend on the order in which particles arrive (bit-reproducible).
+// gather -- the halo box (TX+1)(TY+1)(TZ+4) of each mesh is brought into shared memory by TMA tensor
+//   loads signalled on an mbarrier (tiles touching the upper mesh edge, whose halo wraps periodically,
+//   and meshes whose layout TMA cannot address use plain coalesced row loads); the CTA then interpolates
 //   for the particles of its own tile; results go to out[j] in the caller's particle order.
 #include "pm_internal.cuh"
 
@@ -25,21 +29,134 @@ struct CicGeom {
     int fbits;
     int zs;        // floats per z-row
     long long ms;  // floats per mesh (component stride)
+    int use_tma;   // tensor map valid for this mesh
+    int c0;        // first component (4th tensor-map coordinate)
 };
 
-// the 14 contiguous class runs a tile pulls from itself (m = 0) and its low neighbours
-// m: bit 2/1/0 = neighbour is one tile lower in x/y/z; classes [c0, c1)
-__constant__ signed char kRuns[14][3] = {{0, 0, 8}, {4, 4, 8}, {2, 2, 4}, {2, 6, 8}, {1, 1, 2}, {1, 3, 4}, {1, 5, 6},
-                                         {1, 7, 8}, {6, 6, 8}, {5, 5, 6}, {5, 7, 8}, {3, 3, 4}, {3, 7, 8}, {7, 7, 8}};
-constexpr int NRUNS = 14;
 constexpr int TILE_PTS = TX * TY * TZ;
+constexpr int HX = TX + 1, HY = TY + 1, HZ = TZ + 1;
+constexpr int HZP = TZ + 4;                               // halo row pitch: 144 bytes, a TMA-legal box width
+constexpr int HALO_PTS = HX * HY * HZP;
+constexpr int HALO_STRIDE = (HALO_PTS + 31) / 32 * 32;    // per-mesh stride in shared memory: 128-byte multiple
 
-__device__ __forceinline__ void tile_coords(const CicGeom &g, int tile, int t[3], int t0[3], int ext[3])
+// ---- PTX wrappers: mbarrier + TMA (sm_90+/sm_100a) ----------------------------------------------------
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(unsigned long long *bar, int count)
 {
-    t[2] = tile % g.nt[2];
-    int r = tile / g.nt[2];
-    t[1] = r % g.nt[1];
-    t[0] = r / g.nt[1];
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long *bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned phase)
+{
+    unsigned ok = 0;
+    while (!ok) {
+        asm volatile(
+            "{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+            : "=r"(ok)
+            : "r"(smem_u32(bar)), "r"(phase)
+            : "memory");
+    }
+}
+__device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *m, unsigned long long *bar, int z, int y, int x, int c)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];"
+        ::"r"(smem_u32(dst)), "l"((unsigned long long)m), "r"(smem_u32(bar)), "r"(z), "r"(y), "r"(x), "r"(c)
+        : "memory");
+}
+__device__ __forceinline__ void tma_store_4d(const CUtensorMap *m, const void *src, int z, int y, int x, int c)
+{
+    asm volatile("cp.async.bulk.tensor.4d.global.shared::cta.bulk_group [%0, {%2, %3, %4, %5}], [%1];"
+                 ::"l"((unsigned long long)m), "r"(smem_u32(src)), "r"(z), "r"(y), "r"(x), "r"(c)
+                 : "memory");
+}
+__device__ __forceinline__ void tma_store_commit_and_wait()
+{
+    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+    asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+}
+__device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+// ---- host: tensor maps ------------------------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static EncodeTiledFn encode_fn()
+{
+    static EncodeTiledFn fn = nullptr;
+    static bool tried = false;
+    if (!tried) {
+        tried = true;
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)p;
+        (void)cudaGetLastError();
+    }
+    return fn;
+}
+
+// 4-D view {z, y, x, component} of C meshes [Nx][Ny][zs] spaced ms floats apart; box = {bz, by, bx, 1}
+static bool encode_mesh_map(CUtensorMap *out, const float *base, const int N[3], int C, int zs, long long ms, int bz,
+                            int by, int bx)
+{
+    EncodeTiledFn fn = encode_fn();
+    if (!fn) return false;
+    if (((uintptr_t)base & 15) || (zs & 3) || (ms & 3)) return false;  // 16-byte base and strides
+    cuuint64_t dims[4] = {(cuuint64_t)N[2], (cuuint64_t)N[1], (cuuint64_t)N[0], (cuuint64_t)C};
+    cuuint64_t strides[3] = {(cuuint64_t)zs * 4, (cuuint64_t)zs * 4 * (cuuint64_t)N[1], (cuuint64_t)ms * 4};
+    cuuint32_t box[4] = {(cuuint32_t)bz, (cuuint32_t)by, (cuuint32_t)bx, 1};
+    cuuint32_t estr[4] = {1, 1, 1, 1};
+    CUresult r = fn(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, (void *)base, dims, strides, box, estr,
+                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS;
+}
+
+int cic_init_tensor_maps(pm_ctx *c)
+{
+    const Geometry &g = c->g;
+    c->tma_ok = encode_mesh_map(&c->tmap_load, c->mesh[0], g.N, 7, g.zs, g.mesh_stride, HZP, HY, HX) &&
+                encode_mesh_map(&c->tmap_store, c->mesh[0], g.N, 7, g.zs, g.mesh_stride, TZ, TY, TX);
+    return PM_OK;
+}
+
+// picks the tensor map for a mesh pointer: the ctx's maps for internal meshes, a freshly encoded one otherwise
+static CicGeom make_cic_geom(pm_ctx *c, const float *mesh, int C, int zs, long long ms, bool store, CUtensorMap *map)
+{
+    const Geometry &g = c->g;
+    CicGeom r;
+    for (int d = 0; d < 3; d++) { r.N[d] = g.N[d]; r.nt[d] = g.nt[d]; }
+    r.fbits = g.fbits;
+    r.zs = zs;
+    r.ms = ms;
+    r.use_tma = 0;
+    r.c0 = 0;
+    memset(map, 0, sizeof(*map));
+    long long off = mesh - c->mesh[0];
+    bool internal = zs == g.zs && ms == g.mesh_stride && mesh >= c->mesh[0] && off % g.mesh_stride == 0 &&
+                    off / g.mesh_stride + C <= 7;
+    if (internal && c->tma_ok) {
+        *map = store ? c->tmap_store : c->tmap_load;
+        r.use_tma = 1;
+        r.c0 = (int)(off / g.mesh_stride);
+    } else if (!internal) {
+        if (store ? encode_mesh_map(map, mesh, g.N, C, zs, ms, TZ, TY, TX) : encode_mesh_map(map, mesh, g.N, C, zs, ms, HZP, HY, HX))
+            r.use_tma = 1;
+    }
+    return r;
+}
+
+__device__ __forceinline__ void tile_coords(const CicGeom &g, int t[3], int t0[3], int ext[3])
+{
+    t[0] = blockIdx.z; t[1] = blockIdx.y; t[2] = blockIdx.x;
     t0[0] = t[0] * TX; t0[1] = t[1] * TY; t0[2] = t[2] * TZ;
     ext[0] = min(TX, g.N[0] - t0[0]);
     ext[1] = min(TY, g.N[1] - t0[1]);
@@ -62,121 +179,203 @@ __device__ __forceinline__ float block_sum(float v, float *sh /*>= 32 floats*/)
 // --------------------------------------------------------------------------------------------------
 // scatter
 // --------------------------------------------------------------------------------------------------
+// the 14 contiguous class runs a tile pulls from itself (m = 0) and its low neighbours
+// m: bit 2/1/0 = neighbour is one tile lower in x/y/z; classes [c0, c1)
+__constant__ signed char kRuns[14][3] = {{0, 0, 8}, {4, 4, 8}, {2, 2, 4}, {2, 6, 8}, {1, 1, 2}, {1, 3, 4}, {1, 5, 6},
+                                         {1, 7, 8}, {6, 6, 8}, {5, 5, 6}, {5, 7, 8}, {3, 3, 4}, {3, 7, 8}, {7, 7, 8}};
+constexpr int NRUNS = 14;
+
+// predicated shared-memory integer reduction: no branch, no divergence region around the atomic
+__device__ __forceinline__ void red_shared_if(int *addr, int v, bool ok)
+{
+    asm volatile("{\n .reg .pred p;\n setp.ne.s32 p, %2, 0;\n @p red.shared.add.s32 [%0], %1;\n}"
+                 ::"r"(smem_u32(addr)), "r"(v), "r"((int)ok)
+                 : "memory");
+}
+
+// deposit one particle into the CTA's tile: each of the 8 corners lands only if this tile owns that mesh point
+template <int C>
+__device__ __forceinline__ void deposit(const CicGeom &g, const int t0[3], const int ext[3], uint4 q, const float v[C],
+                                        int (*tile_acc)[TILE_PTS], float fr, unsigned fmask)
+{
+    const unsigned X[3] = {q.x, q.y, q.z};
+    int l[3][2];
+    bool ok[3][2];
+    float w[3][2];
+#pragma unroll
+    for (int d = 0; d < 3; d++) {
+        int l0 = (int)(X[d] >> g.fbits) - t0[d];
+        if (l0 < 0) l0 += g.N[d];          // particle of the low neighbour across the periodic edge
+        int l1 = l0 + 1;
+        if (l1 == g.N[d]) l1 = 0;          // the only tile along d is its own neighbour
+        l[d][0] = l0;
+        l[d][1] = l1;
+        ok[d][0] = l0 < ext[d];
+        ok[d][1] = l1 < ext[d];
+        float td = (float)(X[d] & fmask) * fr;
+        w[d][0] = 1.f - td;
+        w[d][1] = td;
+    }
+#pragma unroll
+    for (int bx = 0; bx < 2; bx++)
+#pragma unroll
+        for (int by = 0; by < 2; by++) {
+            const float wxy = w[0][bx] * w[1][by];
+            const int axy = (l[0][bx] * TY + l[1][by]) * TZ;
+            const bool okxy = ok[0][bx] && ok[1][by];
+#pragma unroll
+            for (int bz = 0; bz < 2; bz++) {
+                const float ww = wxy * w[2][bz];
+                const bool o = okxy && ok[2][bz];
+#pragma unroll
+                for (int c = 0; c < C; c++) red_shared_if(&tile_acc[c][axy + l[2][bz]], __float2int_rn(ww * v[c]), o);
+            }
+        }
+}
+
 template <int C, bool HAS_VAL>
-__global__ void __launch_bounds__(256) scatter_kernel(CicGeom g, const uint4 *__restrict__ rec,
-                                                      const int *__restrict__ offsets,
+__global__ void __launch_bounds__(256) scatter_kernel(const __grid_constant__ CUtensorMap tmap, CicGeom g,
+                                                      const uint4 *__restrict__ rec, const int *__restrict__ offsets,
                                                       const float *__restrict__ val, float *__restrict__ mesh)
 {
-    __shared__ int tile_acc[C][TILE_PTS];
-    __shared__ int run_start[NRUNS];
-    __shared__ int run_prefix[NRUNS + 1];
+    __shared__ __align__(128) int tile_acc[C][TILE_PTS];
+    __shared__ int run_start[NRUNS + 2];
+    __shared__ int run_prefix[NRUNS + 2];
     __shared__ float red[32];
 
     int t[3], t0[3], ext[3];
-    tile_coords(g, blockIdx.x, t, t0, ext);
+    tile_coords(g, t, t0, ext);
 
-    for (int i = threadIdx.x; i < C * TILE_PTS; i += blockDim.x) (&tile_acc[0][0])[i] = 0;
-    if (threadIdx.x < NRUNS) {
-        int m = kRuns[threadIdx.x][0], c0 = kRuns[threadIdx.x][1], c1 = kRuns[threadIdx.x][2];
-        bool valid = true;
-        int n[3];
+    {
+        int4 *z4 = reinterpret_cast<int4 *>(&tile_acc[0][0]);
+        for (int i = threadIdx.x; i < C * TILE_PTS / 4; i += blockDim.x) z4[i] = make_int4(0, 0, 0, 0);
+    }
+    if (threadIdx.x < 32) {
+        const int r = threadIdx.x;
+        int b = 0, len = 0;
+        if (r < NRUNS) {
+            const int m = kRuns[r][0], c0 = kRuns[r][1], c1 = kRuns[r][2];
+            bool valid = true;
+            int n[3];
 #pragma unroll
-        for (int d = 0; d < 3; d++) {
-            int low = (m >> (2 - d)) & 1;
-            if (low && g.nt[d] == 1) valid = false;  // the only tile along d is its own neighbour
-            n[d] = t[d] - low;
-            if (n[d] < 0) n[d] += g.nt[d];
+            for (int d = 0; d < 3; d++) {
+                const int low = (m >> (2 - d)) & 1;
+                if (low && g.nt[d] == 1) valid = false;  // the only tile along d is its own neighbour
+                n[d] = t[d] - low;
+                if (n[d] < 0) n[d] += g.nt[d];
+            }
+            if (valid) {
+                const int key = ((n[0] * g.nt[1] + n[1]) * g.nt[2] + n[2]) * NCLS;
+                b = offsets[key + c0];
+                len = offsets[key + c1] - b;
+            }
         }
-        int key = ((n[0] * g.nt[1] + n[1]) * g.nt[2] + n[2]) * NCLS;
-        int b = 0, e = 0;
-        if (valid) { b = offsets[key + c0]; e = offsets[key + c1]; }
-        run_start[threadIdx.x] = b;
-        run_prefix[threadIdx.x + 1] = e - b;
+        int inc = len;
+#pragma unroll
+        for (int o = 1; o < 16; o <<= 1) {
+            int u = __shfl_up_sync(0xffffffffu, inc, o);
+            if (r >= o) inc += u;
+        }
+        if (r < NRUNS) {
+            run_start[r] = b - (inc - len);  // so that rec index = run_start[r] + flat index
+            run_prefix[r + 1] = inc;
+        }
+        if (r == 0) run_prefix[0] = 0;
     }
     __syncthreads();
-    if (threadIdx.x == 0) {
-        run_prefix[0] = 0;
-        for (int r = 0; r < NRUNS; r++) run_prefix[r + 1] += run_prefix[r];
-    }
-    __syncthreads();
-    const int total = run_prefix[NRUNS];
+    const int own = run_prefix[1], total = run_prefix[NRUNS];
+
+    // flat index -> record (+ values); the own tile is one contiguous run, the 13 neighbour runs are short
+    auto fetch = [&](int i, uint4 &q, float v[C]) {
+        int r = 0;
+        if (i >= own) {
+            r = 1;
+            while (i >= run_prefix[r + 1]) r++;
+        }
+        q = rec[run_start[r] + i];
+        if (HAS_VAL) {
+#pragma unroll
+            for (int c = 0; c < C; c++) v[c] = val[(size_t)q.w * C + c];
+        }
+    };
+
+    // the first two rounds (all of a typical tile) are fetched up front and kept in registers
+    const int i0 = threadIdx.x, i1 = threadIdx.x + blockDim.x;
+    uint4 qa = make_uint4(0, 0, 0, 0), qb = qa;
+    float va[C], vb[C];
+#pragma unroll
+    for (int c = 0; c < C; c++) va[c] = vb[c] = 0.f;
+    if (i0 < total) fetch(i0, qa, va);
+    if (i1 < total) fetch(i1, qb, vb);
 
     // bound on the absolute sum any mesh point can reach -> power-of-two fixed-point scale
     float bound;
     if (HAS_VAL) {
-        float part = 0.f;
-        for (int i = threadIdx.x; i < total; i += blockDim.x) {
-            int r = 0;
-            while (i >= run_prefix[r + 1]) r++;
-            unsigned int j = rec[run_start[r] + (i - run_prefix[r])].w;
+        float ma = 0.f, mb = 0.f;
+#pragma unroll
+        for (int c = 0; c < C; c++) { ma = fmaxf(ma, fabsf(va[c])); mb = fmaxf(mb, fabsf(vb[c])); }
+        float part = ma + mb;
+        for (int i = i1 + blockDim.x; i < total; i += blockDim.x) {
+            uint4 q;
+            float v[C];
+            fetch(i, q, v);
             float m = 0.f;
 #pragma unroll
-            for (int c = 0; c < C; c++) m = fmaxf(m, fabsf(val[(size_t)j * C + c]));
+            for (int c = 0; c < C; c++) m = fmaxf(m, fabsf(v[c]));
             part += m;
         }
         bound = block_sum(part, red) * 1.0001f;  // margin for the fp32 summation itself
     } else {
         bound = (float)total;
     }
-    int ex;
-    frexpf(fmaxf(bound, 1e-37f), &ex);       // bound <= 2^ex
-    int k = min(30 - ex, 96);
-    const float scale = ldexpf(1.f, k), inv_scale = ldexpf(1.f, -k);
+    // bound <= 2^ex with ex from the exponent bits; scale = 2^(30 - ex) capped
+    const int ex = (int)((__float_as_uint(fmaxf(bound, 1e-37f)) >> 23) & 255u) - 126;
+    const int k = min(30 - ex, 96);
+    const float scale = __uint_as_float((unsigned)(127 + k) << 23), inv_scale = __uint_as_float((unsigned)(127 - k) << 23);
     const float fr = 1.f / (float)(1u << g.fbits);
-    const unsigned int fmask = (1u << g.fbits) - 1u;
+    const unsigned fmask = (1u << g.fbits) - 1u;
 
-    for (int i = threadIdx.x; i < total; i += blockDim.x) {
-        int r = 0;
-        while (i >= run_prefix[r + 1]) r++;
-        uint4 q = rec[run_start[r] + (i - run_prefix[r])];
+    auto put = [&](uint4 q, const float vin[C]) {
         float v[C];
-        if (HAS_VAL) {
 #pragma unroll
-            for (int c = 0; c < C; c++) v[c] = val[(size_t)q.w * C + c] * scale;
-        } else {
-#pragma unroll
-            for (int c = 0; c < C; c++) v[c] = scale;
-        }
-        unsigned int X[3] = {q.x, q.y, q.z};
-        int l[3][2];     // local mesh-point index of the two corners per axis, or -1 when not owned
-        float w[3][2];
-#pragma unroll
-        for (int d = 0; d < 3; d++) {
-            int cd = (int)(X[d] >> g.fbits);
-            float td = (float)(X[d] & fmask) * fr;
-            w[d][0] = 1.f - td;
-            w[d][1] = td;
-#pragma unroll
-            for (int b = 0; b < 2; b++) {
-                int gd = cd + b;
-                if (gd == g.N[d]) gd = 0;
-                int ld = gd - t0[d];
-                if (ld < 0) ld += g.N[d];
-                l[d][b] = (ld < ext[d]) ? ld : -1;
-            }
-        }
-#pragma unroll
-        for (int bx = 0; bx < 2; bx++)
-#pragma unroll
-            for (int by = 0; by < 2; by++)
-#pragma unroll
-                for (int bz = 0; bz < 2; bz++) {
-                    if ((l[0][bx] | l[1][by] | l[2][bz]) < 0) continue;
-                    float ww = w[0][bx] * w[1][by] * w[2][bz];
-                    int idx = (l[0][bx] * TY + l[1][by]) * TZ + l[2][bz];
-#pragma unroll
-                    for (int c = 0; c < C; c++) atomicAdd(&tile_acc[c][idx], __float2int_rn(ww * v[c]));
-                }
+        for (int c = 0; c < C; c++) v[c] = HAS_VAL ? vin[c] * scale : scale;
+        deposit<C>(g, t0, ext, q, v, tile_acc, fr, fmask);
+    };
+    if (i0 < total) put(qa, va);
+    if (i1 < total) put(qb, vb);
+    for (int i = i1 + blockDim.x; i < total; i += blockDim.x) {
+        uint4 q;
+        float v[C];
+        fetch(i, q, v);
+        put(q, v);
     }
     __syncthreads();
 
-    for (int i = threadIdx.x; i < TILE_PTS; i += blockDim.x) {
-        int lz = i % TZ, r = i / TZ;
-        int ly = r % TY, lx = r / TY;
-        if (lx < ext[0] && ly < ext[1] && lz < ext[2]) {
-            size_t o = ((size_t)(t0[0] + lx) * g.N[1] + (t0[1] + ly)) * g.zs + (t0[2] + lz);
+    if (g.use_tma) {
+        // int -> float in place (same bytes), then one tensor store per component; TMA clips at the mesh edge
+        int4 *a4 = reinterpret_cast<int4 *>(&tile_acc[0][0]);
+        for (int i = threadIdx.x; i < C * TILE_PTS / 4; i += blockDim.x) {
+            int4 a = a4[i];
+            float4 f = make_float4((float)a.x * inv_scale, (float)a.y * inv_scale, (float)a.z * inv_scale, (float)a.w * inv_scale);
+            reinterpret_cast<float4 *>(a4)[i] = f;
+        }
+        fence_proxy_async_smem();
+        __syncthreads();
+        if (threadIdx.x == 0) {
 #pragma unroll
-            for (int c = 0; c < C; c++) mesh[(size_t)c * g.ms + o] = (float)tile_acc[c][i] * inv_scale;
+            for (int c = 0; c < C; c++) tma_store_4d(&tmap, &tile_acc[c][0], t0[2], t0[1], t0[0], g.c0 + c);
+            tma_store_commit_and_wait();
+        }
+    } else {
+        // plain path: one warp per z-row
+        const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = blockDim.x >> 5;
+        for (int row = w; row < TX * TY; row += nw) {
+            const int lx = row / TY, ly = row % TY;
+            if (lx < ext[0] && ly < ext[1] && lane < ext[2]) {
+                const size_t o = ((size_t)(t0[0] + lx) * g.N[1] + (t0[1] + ly)) * g.zs + (t0[2] + lane);
+#pragma unroll
+                for (int c = 0; c < C; c++) mesh[(size_t)c * g.ms + o] = (float)tile_acc[c][row * TZ + lane] * inv_scale;
+            }
         }
     }
 }
@@ -184,43 +383,67 @@ __global__ void __launch_bounds__(256) scatter_kernel(CicGeom g, const uint4 *__
 // --------------------------------------------------------------------------------------------------
 // gathers
 // --------------------------------------------------------------------------------------------------
-constexpr int HX = TX + 1, HY = TY + 1, HZ = TZ + 1;
-constexpr int HALO_PTS = HX * HY * HZ;
 enum GatherMode { G_VALUE = 0, G_GRAD = 1, G_FUSED = 2 };
 
 template <int C, int MODE, bool HAS_COT>
-__global__ void __launch_bounds__(256) gather_kernel(CicGeom g, const uint4 *__restrict__ rec,
-                                                     const int *__restrict__ offsets,
+__global__ void __launch_bounds__(256) gather_kernel(const __grid_constant__ CUtensorMap tmap, CicGeom g,
+                                                     const uint4 *__restrict__ rec, const int *__restrict__ offsets,
                                                      const float *__restrict__ mesh, const float *__restrict__ cot,
                                                      float cot_scale, float *__restrict__ out, float *__restrict__ out2)
 {
-    __shared__ float halo[C][HALO_PTS];
+    __shared__ __align__(128) float halo[C * HALO_STRIDE];
+    __shared__ __align__(8) unsigned long long bar;
     int t[3], t0[3], ext[3];
-    tile_coords(g, blockIdx.x, t, t0, ext);
-    const int key0 = blockIdx.x * NCLS;
+    tile_coords(g, t, t0, ext);
+    const int key0 = ((t[0] * g.nt[1] + t[1]) * g.nt[2] + t[2]) * NCLS;
     const int beg = offsets[key0], end = offsets[key0 + NCLS];
     if (beg == end) return;
 
-    for (int i = threadIdx.x; i < HALO_PTS; i += blockDim.x) {
-        int lz = i % HZ, r = i / HZ;
-        int ly = r % HY, lx = r / HY;
-        if (lx <= ext[0] && ly <= ext[1] && lz <= ext[2]) {
-            int gx = t0[0] + lx, gy = t0[1] + ly, gz = t0[2] + lz;
-            if (gx >= g.N[0]) gx -= g.N[0];
-            if (gy >= g.N[1]) gy -= g.N[1];
-            if (gz >= g.N[2]) gz -= g.N[2];
-            size_t o = ((size_t)gx * g.N[1] + gy) * g.zs + gz;
+    // the halo reaches one point past the tile: interior tiles never wrap and can take the TMA box as is
+    const bool interior = g.use_tma && t0[0] + ext[0] < g.N[0] && t0[1] + ext[1] < g.N[1] && t0[2] + ext[2] < g.N[2];
+    uint4 q = make_uint4(0, 0, 0, 0);
+    if (interior) {
+        if (threadIdx.x == 0) mbar_init(&bar, 1);
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            mbar_expect_tx(&bar, (unsigned)(C * HALO_PTS * sizeof(float)));
 #pragma unroll
-            for (int c = 0; c < C; c++) halo[c][i] = mesh[(size_t)c * g.ms + o];
+            for (int c = 0; c < C; c++) tma_load_4d(&halo[c * HALO_STRIDE], &tmap, &bar, t0[2], t0[1], t0[0], g.c0 + c);
         }
+        if (beg + (int)threadIdx.x < end) q = rec[beg + threadIdx.x];  // overlaps the TMA flight
+        mbar_wait(&bar, 0);
+    } else {
+        const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = blockDim.x >> 5;
+        for (int row = w; row < C * HX * HY; row += nw) {
+            const int c = row / (HX * HY), r2 = row % (HX * HY);
+            const int lx = r2 / HY, ly = r2 % HY;
+            if (lx <= ext[0] && ly <= ext[1]) {
+                int gx = t0[0] + lx, gy = t0[1] + ly;
+                if (gx >= g.N[0]) gx -= g.N[0];
+                if (gy >= g.N[1]) gy -= g.N[1];
+                const float *src = mesh + (size_t)c * g.ms + ((size_t)gx * g.N[1] + gy) * g.zs;
+                float *dst = &halo[c * HALO_STRIDE + (lx * HY + ly) * HZP];
+                if (lane <= ext[2]) {
+                    int gz = t0[2] + lane;
+                    if (gz >= g.N[2]) gz -= g.N[2];
+                    dst[lane] = src[gz];
+                }
+                if (lane == 0 && ext[2] == TZ) {
+                    int gz = t0[2] + TZ;
+                    if (gz >= g.N[2]) gz -= g.N[2];
+                    dst[TZ] = src[gz];
+                }
+            }
+        }
+        if (beg + (int)threadIdx.x < end) q = rec[beg + threadIdx.x];
+        __syncthreads();
     }
-    __syncthreads();
 
     const float fr = 1.f / (float)(1u << g.fbits);
-    const unsigned int fmask = (1u << g.fbits) - 1u;
+    const unsigned fmask = (1u << g.fbits) - 1u;
     for (int i = beg + threadIdx.x; i < end; i += blockDim.x) {
-        uint4 q = rec[i];
-        unsigned int X[3] = {q.x, q.y, q.z};
+        if (i != beg + (int)threadIdx.x) q = rec[i];
+        const unsigned X[3] = {q.x, q.y, q.z};
         int l[3];
         float w[3][2];
 #pragma unroll
@@ -230,7 +453,7 @@ __global__ void __launch_bounds__(256) gather_kernel(CicGeom g, const uint4 *__r
             w[d][0] = 1.f - td;
             w[d][1] = td;
         }
-        const int base = (l[0] * HY + l[1]) * HZ + l[2];
+        const int base = (l[0] * HY + l[1]) * HZP + l[2];
         const size_t j = q.w;
         float cv[C];
         if (MODE == G_GRAD) {
@@ -252,7 +475,7 @@ __global__ void __launch_bounds__(256) gather_kernel(CicGeom g, const uint4 *__r
             for (int by = 0; by < 2; by++)
 #pragma unroll
                 for (int bz = 0; bz < 2; bz++) {
-                    const int idx = base + (bx * HY + by) * HZ + bz;
+                    const int idx = base + (bx * HY + by) * HZP + bz;
                     const float W = w[0][bx] * w[1][by] * w[2][bz];
                     const float dWx = (bx ? 1.f : -1.f) * w[1][by] * w[2][bz];
                     const float dWy = (by ? 1.f : -1.f) * w[0][bx] * w[2][bz];
@@ -260,7 +483,7 @@ __global__ void __launch_bounds__(256) gather_kernel(CicGeom g, const uint4 *__r
                     float m = 0.f;  // cotangent-weighted mesh value at this corner
 #pragma unroll
                     for (int c = 0; c < C; c++) {
-                        float f = halo[c][idx];
+                        const float f = halo[c * HALO_STRIDE + idx];
                         if (MODE != G_GRAD) val[c] += W * f;
                         if (MODE != G_VALUE) m += cv[c] * f;
                     }
@@ -286,33 +509,27 @@ __global__ void __launch_bounds__(256) gather_kernel(CicGeom g, const uint4 *__r
     }
 }
 
-static CicGeom make_cic_geom(const Geometry &g, int zs, long long ms)
-{
-    CicGeom c;
-    for (int d = 0; d < 3; d++) { c.N[d] = g.N[d]; c.nt[d] = g.nt[d]; }
-    c.fbits = g.fbits;
-    c.zs = zs;
-    c.ms = ms;
-    return c;
-}
+static dim3 tile_grid(const Geometry &g) { return dim3((unsigned)g.nt[2], (unsigned)g.nt[1], (unsigned)g.nt[0]); }
 
 int scatter_sorted(pm_ctx *c, const float *val, int C, float *mesh, int zs, long long ms)
 {
-    CicGeom g = make_cic_geom(c->g, zs, ms);
-    double np = (double)c->g.np, ng = (double)c->g.ng;
+    CUtensorMap map;
+    CicGeom g = make_cic_geom(c, mesh, C, zs, ms, true, &map);
+    double np = (double)c->cur_np, ng = (double)c->g.ng;
+    dim3 grid = tile_grid(c->g);
     if (C == 1 && !val) {
         Timer t(c, TC_SCATTER1, 12.0 * np + 4.0 * ng);
-        scatter_kernel<1, false><<<c->g.ntiles, 256, 0, c->stream>>>(g, c->rec, c->offsets, nullptr, mesh);
+        scatter_kernel<1, false><<<grid, 256, 0, c->stream>>>(map, g, c->rec, c->offsets, nullptr, mesh);
         PM_LAUNCH_CHECK(c, "scatter_kernel<1>");
         t.stop();
     } else if (C == 1) {
         Timer t(c, TC_SCATTER1, 16.0 * np + 4.0 * ng);
-        scatter_kernel<1, true><<<c->g.ntiles, 256, 0, c->stream>>>(g, c->rec, c->offsets, val, mesh);
+        scatter_kernel<1, true><<<grid, 256, 0, c->stream>>>(map, g, c->rec, c->offsets, val, mesh);
         PM_LAUNCH_CHECK(c, "scatter_kernel<1,val>");
         t.stop();
     } else if (C == 3 && val) {
         Timer t(c, TC_SCATTER3, 24.0 * np + 12.0 * ng);
-        scatter_kernel<3, true><<<c->g.ntiles, 256, 0, c->stream>>>(g, c->rec, c->offsets, val, mesh);
+        scatter_kernel<3, true><<<grid, 256, 0, c->stream>>>(map, g, c->rec, c->offsets, val, mesh);
         PM_LAUNCH_CHECK(c, "scatter_kernel<3,val>");
         t.stop();
     } else {
@@ -323,16 +540,18 @@ int scatter_sorted(pm_ctx *c, const float *val, int C, float *mesh, int zs, long
 
 int gather_sorted(pm_ctx *c, const float *mesh, int C, int zs, long long ms, float *out)
 {
-    CicGeom g = make_cic_geom(c->g, zs, ms);
-    double np = (double)c->g.np, ng = (double)c->g.ng;
+    CUtensorMap map;
+    CicGeom g = make_cic_geom(c, mesh, C, zs, ms, false, &map);
+    double np = (double)c->cur_np, ng = (double)c->g.ng;
+    dim3 grid = tile_grid(c->g);
     if (C == 1) {
         Timer t(c, TC_GATHER3, 16.0 * np + 4.0 * ng);
-        gather_kernel<1, G_VALUE, false><<<c->g.ntiles, 256, 0, c->stream>>>(g, c->rec, c->offsets, mesh, nullptr, 1.f, out, nullptr);
+        gather_kernel<1, G_VALUE, false><<<grid, 256, 0, c->stream>>>(map, g, c->rec, c->offsets, mesh, nullptr, 1.f, out, nullptr);
         PM_LAUNCH_CHECK(c, "gather_kernel<1>");
         t.stop();
     } else if (C == 3) {
         Timer t(c, TC_GATHER3, 24.0 * np + 12.0 * ng);
-        gather_kernel<3, G_VALUE, false><<<c->g.ntiles, 256, 0, c->stream>>>(g, c->rec, c->offsets, mesh, nullptr, 1.f, out, nullptr);
+        gather_kernel<3, G_VALUE, false><<<grid, 256, 0, c->stream>>>(map, g, c->rec, c->offsets, mesh, nullptr, 1.f, out, nullptr);
         PM_LAUNCH_CHECK(c, "gather_kernel<3>");
         t.stop();
     } else {
@@ -344,17 +563,19 @@ int gather_sorted(pm_ctx *c, const float *mesh, int C, int zs, long long ms, flo
 int gather_grad_sorted(pm_ctx *c, const float *mesh, int C, int zs, long long ms, const float *cot, float cot_scale,
                        float *out)
 {
-    CicGeom g = make_cic_geom(c->g, zs, ms);
-    double np = (double)c->g.np, ng = (double)c->g.ng;
+    CUtensorMap map;
+    CicGeom g = make_cic_geom(c, mesh, C, zs, ms, false, &map);
+    double np = (double)c->cur_np, ng = (double)c->g.ng;
+    dim3 grid = tile_grid(c->g);
     Timer t(c, TC_GATHER_GRAD, (24.0 + (cot ? 4.0 * C : 0.0)) * np + 4.0 * C * ng);
     if (C == 1 && !cot)
-        gather_kernel<1, G_GRAD, false><<<c->g.ntiles, 256, 0, c->stream>>>(g, c->rec, c->offsets, mesh, nullptr, cot_scale, out, nullptr);
+        gather_kernel<1, G_GRAD, false><<<grid, 256, 0, c->stream>>>(map, g, c->rec, c->offsets, mesh, nullptr, cot_scale, out, nullptr);
     else if (C == 1)
-        gather_kernel<1, G_GRAD, true><<<c->g.ntiles, 256, 0, c->stream>>>(g, c->rec, c->offsets, mesh, cot, cot_scale, out, nullptr);
+        gather_kernel<1, G_GRAD, true><<<grid, 256, 0, c->stream>>>(map, g, c->rec, c->offsets, mesh, cot, cot_scale, out, nullptr);
     else if (C == 3 && !cot)
-        gather_kernel<3, G_GRAD, false><<<c->g.ntiles, 256, 0, c->stream>>>(g, c->rec, c->offsets, mesh, nullptr, cot_scale, out, nullptr);
+        gather_kernel<3, G_GRAD, false><<<grid, 256, 0, c->stream>>>(map, g, c->rec, c->offsets, mesh, nullptr, cot_scale, out, nullptr);
     else if (C == 3)
-        gather_kernel<3, G_GRAD, true><<<c->g.ntiles, 256, 0, c->stream>>>(g, c->rec, c->offsets, mesh, cot, cot_scale, out, nullptr);
+        gather_kernel<3, G_GRAD, true><<<grid, 256, 0, c->stream>>>(map, g, c->rec, c->offsets, mesh, cot, cot_scale, out, nullptr);
     else
         return fail(c, PM_EINVAL, "gather_grad", "C must be 1 or 3");
     PM_LAUNCH_CHECK(c, "gather_kernel<grad>");
@@ -364,10 +585,11 @@ int gather_grad_sorted(pm_ctx *c, const float *mesh, int C, int zs, long long ms
 
 int gather_fused_sorted(pm_ctx *c, const float *mesh4, int zs, long long ms, const float *pi, float *acc, float *alpha)
 {
-    CicGeom g = make_cic_geom(c->g, zs, ms);
-    double np = (double)c->g.np, ng = (double)c->g.ng;
+    CUtensorMap map;
+    CicGeom g = make_cic_geom(c, mesh4, 4, zs, ms, false, &map);
+    double np = (double)c->cur_np, ng = (double)c->g.ng;
     Timer t(c, TC_GATHER_FUSED, 48.0 * np + 16.0 * ng);
-    gather_kernel<4, G_FUSED, true><<<c->g.ntiles, 256, 0, c->stream>>>(g, c->rec, c->offsets, mesh4, pi, 1.f, acc, alpha);
+    gather_kernel<4, G_FUSED, true><<<tile_grid(c->g), 256, 0, c->stream>>>(map, g, c->rec, c->offsets, mesh4, pi, 1.f, acc, alpha);
     PM_LAUNCH_CHECK(c, "gather_kernel<fused>");
     t.stop();
     return PM_OK;

@@ -1,6 +1,7 @@
 // pm_internal.cuh -- private declarations of libpm (CUDA, sm_100a).  Not part of the ABI.
 // Shares nothing with oracle/ (the CPU fp64 oracle is test infrastructure with its own code).
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <cufft.h>
 #include <stdint.h>
@@ -51,7 +52,8 @@ struct Geometry {
     int L[3];        // lattice
     int nt[3];       // tiles per axis
     int fbits;       // fraction bits of the absolute fixed-point coordinate
-    int zs;          // floats per z-row of a (padded) internal mesh: Nz + 2
+    int zs;          // floats per z-row of a (padded) internal mesh: Nz + 2 rounded up to a multiple of 4
+                     // (16-byte rows: TMA global strides and vector loads need it; cuFFT takes it as inembed)
     long long np;    // particles of the lattice
     long long ng;    // Nx*Ny*Nz
     long long mesh_stride;  // floats per internal padded mesh: Nx*Ny*(Nz+2)
@@ -85,6 +87,8 @@ struct pm_ctx {
     float *ktab;                 // [3 axes][3: kt, k^2, dec][ktabn] per-axis k-space tables
     int ktabn;
     long long cur_np;            // particles in the current sort
+    CUtensorMap tmap_load, tmap_store;  // 4-D {z, y, x, mesh 0..6} views of the internal meshes: halo box / tile box
+    bool tma_ok;                 // cuTensorMapEncodeTiled resolved and the internal maps encoded
     void *fft_work;
     size_t fft_work_bytes;
     // integrator bookkeeping
@@ -138,7 +142,11 @@ double kick_factor_host(double om, double ac, double aa, double ab);
 int bin_particles(pm_ctx *c, long long np, const float *x);
 
 // ---- CIC (pm_cic.cu): operate on the sorted records of the last bin_particles -----------------------
+// encode the two internal tensor maps (call once from pm_init); failure leaves tma_ok = false (plain loads)
+int cic_init_tensor_maps(pm_ctx *c);
 // val: [np][C] in ORIGINAL particle order or NULL.  mesh: C meshes, row stride zs, mesh stride ms.
+// Internal meshes (pointers inside c->mesh[]) use the ctx's tensor maps; other pointers get a map encoded per call
+// when their layout allows TMA (16-byte aligned base and strides), else the kernels' plain load/store path.
 int scatter_sorted(pm_ctx *c, const float *val, int C, float *mesh, int zs, long long ms);
 int gather_sorted(pm_ctx *c, const float *mesh, int C, int zs, long long ms, float *out);
 int gather_grad_sorted(pm_ctx *c, const float *mesh, int C, int zs, long long ms, const float *cot,

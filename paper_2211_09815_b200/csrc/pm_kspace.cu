@@ -13,7 +13,8 @@ namespace pm {
 
 struct KGeom {
     int N[3];
-    int nzc;            // Nz/2 + 1
+    int nzc;            // Nz/2 + 1 modes per z-row
+    int zsc;            // complex elements per (padded) z-row in memory: zs / 2
     long long nk;       // complex elements per mesh
     long long cstride;  // complex elements between components (padded mesh stride / 2)
     const float *tab;   // [3 axes][3: kt, k2, dec][tabn]
@@ -21,7 +22,8 @@ struct KGeom {
     float c0;           // 3/2 Om / (nbar N_g)
 };
 
-__device__ __forceinline__ void k_factors(const KGeom &g, long long idx, float kt[3], float *G)
+// idx enumerates the Nx*Ny*(Nz/2+1) modes; returns the element offset of that mode in the padded mesh
+__device__ __forceinline__ size_t k_factors(const KGeom &g, long long idx, float kt[3], float *G)
 {
     int iz = (int)(idx % g.nzc);
     long long row = idx / g.nzc;
@@ -34,6 +36,7 @@ __device__ __forceinline__ void k_factors(const KGeom &g, long long idx, float k
     float k2 = tx[g.tabn + ix] + ty[g.tabn + iy] + tz[g.tabn + iz];
     float dec = tx[2 * g.tabn + ix] * ty[2 * g.tabn + iy] * tz[2 * g.tabn + iz];
     *G = (ix | iy | iz) == 0 ? 0.f : g.c0 * dec / k2;
+    return (size_t)row * g.zsc + iz;
 }
 
 __global__ void __launch_bounds__(256) kspace_force_kernel(KGeom g, const float2 *__restrict__ rho_k, float2 *__restrict__ f_k)
@@ -41,12 +44,12 @@ __global__ void __launch_bounds__(256) kspace_force_kernel(KGeom g, const float2
     long long stride = (long long)gridDim.x * blockDim.x;
     for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < g.nk; idx += stride) {
         float kt[3], G;
-        k_factors(g, idx, kt, &G);
-        float2 r = rho_k[idx];
+        size_t o = k_factors(g, idx, kt, &G);
+        float2 r = rho_k[o];
 #pragma unroll
         for (int d = 0; d < 3; d++) {
             float c = kt[d] * G;  // times +i: (re, im) -> (-c im, c re)
-            f_k[(size_t)d * g.cstride + idx] = make_float2(-c * r.y, c * r.x);
+            f_k[(size_t)d * g.cstride + o] = make_float2(-c * r.y, c * r.x);
         }
     }
 }
@@ -56,16 +59,16 @@ __global__ void __launch_bounds__(256) kspace_adjoint_kernel(KGeom g, const floa
     long long stride = (long long)gridDim.x * blockDim.x;
     for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < g.nk; idx += stride) {
         float kt[3], G;
-        k_factors(g, idx, kt, &G);
+        size_t o = k_factors(g, idx, kt, &G);
         float re = 0.f, im = 0.f;
 #pragma unroll
         for (int d = 0; d < 3; d++) {
-            float2 v = Pi_k[(size_t)d * g.cstride + idx];
+            float2 v = Pi_k[(size_t)d * g.cstride + o];
             re += kt[d] * v.x;
             im += kt[d] * v.y;
         }
         // times -i G: (re, im) -> (G im, -G re)
-        psi_k[idx] = make_float2(G * im, -G * re);
+        psi_k[o] = make_float2(G * im, -G * re);
     }
 }
 
@@ -74,6 +77,7 @@ static KGeom make_kgeom(pm_ctx *c, double nbar)
     KGeom k;
     for (int d = 0; d < 3; d++) k.N[d] = c->g.N[d];
     k.nzc = c->g.N[2] / 2 + 1;
+    k.zsc = c->g.zs / 2;
     k.nk = c->g.nk;
     k.cstride = c->g.mesh_stride / 2;
     k.tab = c->ktab;
