@@ -20,6 +20,8 @@
 //   loads signalled on an mbarrier (tiles touching the upper mesh edge, whose halo wraps periodically,
 //   and meshes whose layout TMA cannot address use plain coalesced row loads); the CTA then interpolates
 //   for the particles of its own tile; results go to out[j] in the caller's particle order.
+#include <cstdlib>
+
 #include "pm_internal.cuh"
 
 namespace pm {
@@ -31,6 +33,7 @@ struct CicGeom {
     long long ms;  // floats per mesh (component stride)
     int use_tma;   // tensor map valid for this mesh
     int c0;        // first component (4th tensor-map coordinate)
+    int kshift;    // debug: coarsen the scatter's fixed-point scale by this many bits (0 in production)
 };
 
 constexpr int TILE_PTS = TX * TY * TZ;
@@ -139,6 +142,7 @@ static CicGeom make_cic_geom(pm_ctx *c, const float *mesh, int C, int zs, long l
     r.ms = ms;
     r.use_tma = 0;
     r.c0 = 0;
+    { const char *e = getenv("PM_DEBUG_KSHIFT"); r.kshift = e ? atoi(e) : 0; }
     memset(map, 0, sizeof(*map));
     long long off = mesh - c->mesh[0];
     bool internal = zs == g.zs && ms == g.mesh_stride && mesh >= c->mesh[0] && off % g.mesh_stride == 0 &&
@@ -194,7 +198,7 @@ __device__ __forceinline__ void red_shared_if(int *addr, int v, bool ok)
 }
 
 // deposit one particle into the CTA's tile: each of the 8 corners lands only if this tile owns that mesh point
-template <int C>
+template <int C, bool SIGNED>
 __device__ __forceinline__ void deposit(const CicGeom &g, const int t0[3], const int ext[3], uint4 q, const float v[C],
                                         int (*tile_acc)[TILE_PTS], float fr, unsigned fmask)
 {
@@ -228,7 +232,8 @@ __device__ __forceinline__ void deposit(const CicGeom &g, const int t0[3], const
                 const float ww = wxy * w[2][bz];
                 const bool o = okxy && ok[2][bz];
 #pragma unroll
-                for (int c = 0; c < C; c++) red_shared_if(&tile_acc[c][axy + l[2][bz]], __float2int_rn(ww * v[c]), o);
+                for (int c = 0; c < C; c++)
+                    red_shared_if(&tile_acc[c][axy + l[2][bz]], SIGNED ? __float2int_rn(ww * v[c]) : (int)__float2uint_rn(ww * v[c]), o);
             }
         }
 }
@@ -328,10 +333,23 @@ __global__ void __launch_bounds__(256) scatter_kernel(const __grid_constant__ CU
     } else {
         bound = (float)total;
     }
-    // bound <= 2^ex with ex from the exponent bits; scale = 2^(30 - ex) capped
-    const int ex = (int)((__float_as_uint(fmaxf(bound, 1e-37f)) >> 23) & 255u) - 126;
-    const int k = min(30 - ex, 96);
-    const float scale = __uint_as_float((unsigned)(127 + k) << 23), inv_scale = __uint_as_float((unsigned)(127 - k) << 23);
+    // fixed-point scale: the accumulators cannot overflow because |sum at any point| <= bound, and each of the
+    // <= total deposits at a point rounds by <= 0.5.
+    //   unit mass: deposits are >= 0 -> UNSIGNED accumulation with scale = (2^32 - headroom) / total.  total is an
+    //              integer, so the scale (not a power of two: one extra fp32 rounding per deposit, 6e-8 relative,
+    //              far below the quantum) is the same in every run: the density mesh stays bit-reproducible.
+    //   values:    signed accumulation; bound is an fp32 sum whose last bits depend on the (arbitrary) order of
+    //              the records, so only its exponent is used: scale = 2^(30 - ex) with bound <= 2^ex.
+    float scale;
+    if (HAS_VAL) {
+        const int ex = (int)((__float_as_uint(fmaxf(bound, 1e-37f)) >> 23) & 255u) - 126;
+        const int k = min(30 - ex, 96) - g.kshift;
+        scale = __uint_as_float((unsigned)(127 + k) << 23);
+    } else {
+        const float room = fmaxf(4294967296.f * 0.99999f - (float)total, 1.f);
+        scale = ldexpf(room / fmaxf(bound, 1.f), -g.kshift);
+    }
+    const float inv_scale = 1.f / scale;
     const float fr = 1.f / (float)(1u << g.fbits);
     const unsigned fmask = (1u << g.fbits) - 1u;
 
@@ -339,7 +357,7 @@ __global__ void __launch_bounds__(256) scatter_kernel(const __grid_constant__ CU
         float v[C];
 #pragma unroll
         for (int c = 0; c < C; c++) v[c] = HAS_VAL ? vin[c] * scale : scale;
-        deposit<C>(g, t0, ext, q, v, tile_acc, fr, fmask);
+        deposit<C, HAS_VAL>(g, t0, ext, q, v, tile_acc, fr, fmask);
     };
     if (i0 < total) put(qa, va);
     if (i1 < total) put(qb, vb);
@@ -356,7 +374,9 @@ __global__ void __launch_bounds__(256) scatter_kernel(const __grid_constant__ CU
         int4 *a4 = reinterpret_cast<int4 *>(&tile_acc[0][0]);
         for (int i = threadIdx.x; i < C * TILE_PTS / 4; i += blockDim.x) {
             int4 a = a4[i];
-            float4 f = make_float4((float)a.x * inv_scale, (float)a.y * inv_scale, (float)a.z * inv_scale, (float)a.w * inv_scale);
+            float4 f = HAS_VAL ? make_float4((float)a.x * inv_scale, (float)a.y * inv_scale, (float)a.z * inv_scale, (float)a.w * inv_scale)
+                               : make_float4((float)(unsigned)a.x * inv_scale, (float)(unsigned)a.y * inv_scale,
+                                             (float)(unsigned)a.z * inv_scale, (float)(unsigned)a.w * inv_scale);
             reinterpret_cast<float4 *>(a4)[i] = f;
         }
         fence_proxy_async_smem();
@@ -374,7 +394,10 @@ __global__ void __launch_bounds__(256) scatter_kernel(const __grid_constant__ CU
             if (lx < ext[0] && ly < ext[1] && lane < ext[2]) {
                 const size_t o = ((size_t)(t0[0] + lx) * g.N[1] + (t0[1] + ly)) * g.zs + (t0[2] + lane);
 #pragma unroll
-                for (int c = 0; c < C; c++) mesh[(size_t)c * g.ms + o] = (float)tile_acc[c][row * TZ + lane] * inv_scale;
+                for (int c = 0; c < C; c++) {
+                    const int a = tile_acc[c][row * TZ + lane];
+                    mesh[(size_t)c * g.ms + o] = (HAS_VAL ? (float)a : (float)(unsigned)a) * inv_scale;
+                }
             }
         }
     }
@@ -510,6 +533,12 @@ __global__ void __launch_bounds__(256) gather_kernel(const __grid_constant__ CUt
 }
 
 static dim3 tile_grid(const Geometry &g) { return dim3((unsigned)g.nt[2], (unsigned)g.nt[1], (unsigned)g.nt[0]); }
+static int env_threads(const char *name, int dflt)
+{
+    const char *e = getenv(name);
+    int v = e ? atoi(e) : dflt;
+    return (v >= 32 && v <= 256 && v % 32 == 0) ? v : dflt;
+}
 
 int scatter_sorted(pm_ctx *c, const float *val, int C, float *mesh, int zs, long long ms)
 {
@@ -519,17 +548,17 @@ int scatter_sorted(pm_ctx *c, const float *val, int C, float *mesh, int zs, long
     dim3 grid = tile_grid(c->g);
     if (C == 1 && !val) {
         Timer t(c, TC_SCATTER1, 12.0 * np + 4.0 * ng);
-        scatter_kernel<1, false><<<grid, 256, 0, c->stream>>>(map, g, c->rec, c->offsets, nullptr, mesh);
+        scatter_kernel<1, false><<<grid, env_threads("PM_SCATTER_THREADS", 128), 0, c->stream>>>(map, g, c->rec, c->offsets, nullptr, mesh);
         PM_LAUNCH_CHECK(c, "scatter_kernel<1>");
         t.stop();
     } else if (C == 1) {
         Timer t(c, TC_SCATTER1, 16.0 * np + 4.0 * ng);
-        scatter_kernel<1, true><<<grid, 256, 0, c->stream>>>(map, g, c->rec, c->offsets, val, mesh);
+        scatter_kernel<1, true><<<grid, env_threads("PM_SCATTER_THREADS", 128), 0, c->stream>>>(map, g, c->rec, c->offsets, val, mesh);
         PM_LAUNCH_CHECK(c, "scatter_kernel<1,val>");
         t.stop();
     } else if (C == 3 && val) {
         Timer t(c, TC_SCATTER3, 24.0 * np + 12.0 * ng);
-        scatter_kernel<3, true><<<grid, 256, 0, c->stream>>>(map, g, c->rec, c->offsets, val, mesh);
+        scatter_kernel<3, true><<<grid, env_threads("PM_SCATTER_THREADS", 256), 0, c->stream>>>(map, g, c->rec, c->offsets, val, mesh);
         PM_LAUNCH_CHECK(c, "scatter_kernel<3,val>");
         t.stop();
     } else {
@@ -546,12 +575,12 @@ int gather_sorted(pm_ctx *c, const float *mesh, int C, int zs, long long ms, flo
     dim3 grid = tile_grid(c->g);
     if (C == 1) {
         Timer t(c, TC_GATHER3, 16.0 * np + 4.0 * ng);
-        gather_kernel<1, G_VALUE, false><<<grid, 256, 0, c->stream>>>(map, g, c->rec, c->offsets, mesh, nullptr, 1.f, out, nullptr);
+        gather_kernel<1, G_VALUE, false><<<grid, env_threads("PM_GATHER_THREADS", 256), 0, c->stream>>>(map, g, c->rec, c->offsets, mesh, nullptr, 1.f, out, nullptr);
         PM_LAUNCH_CHECK(c, "gather_kernel<1>");
         t.stop();
     } else if (C == 3) {
         Timer t(c, TC_GATHER3, 24.0 * np + 12.0 * ng);
-        gather_kernel<3, G_VALUE, false><<<grid, 256, 0, c->stream>>>(map, g, c->rec, c->offsets, mesh, nullptr, 1.f, out, nullptr);
+        gather_kernel<3, G_VALUE, false><<<grid, env_threads("PM_GATHER_THREADS", 256), 0, c->stream>>>(map, g, c->rec, c->offsets, mesh, nullptr, 1.f, out, nullptr);
         PM_LAUNCH_CHECK(c, "gather_kernel<3>");
         t.stop();
     } else {
@@ -569,13 +598,13 @@ int gather_grad_sorted(pm_ctx *c, const float *mesh, int C, int zs, long long ms
     dim3 grid = tile_grid(c->g);
     Timer t(c, TC_GATHER_GRAD, (24.0 + (cot ? 4.0 * C : 0.0)) * np + 4.0 * C * ng);
     if (C == 1 && !cot)
-        gather_kernel<1, G_GRAD, false><<<grid, 256, 0, c->stream>>>(map, g, c->rec, c->offsets, mesh, nullptr, cot_scale, out, nullptr);
+        gather_kernel<1, G_GRAD, false><<<grid, env_threads("PM_GATHER_THREADS", 256), 0, c->stream>>>(map, g, c->rec, c->offsets, mesh, nullptr, cot_scale, out, nullptr);
     else if (C == 1)
-        gather_kernel<1, G_GRAD, true><<<grid, 256, 0, c->stream>>>(map, g, c->rec, c->offsets, mesh, cot, cot_scale, out, nullptr);
+        gather_kernel<1, G_GRAD, true><<<grid, env_threads("PM_GATHER_THREADS", 256), 0, c->stream>>>(map, g, c->rec, c->offsets, mesh, cot, cot_scale, out, nullptr);
     else if (C == 3 && !cot)
-        gather_kernel<3, G_GRAD, false><<<grid, 256, 0, c->stream>>>(map, g, c->rec, c->offsets, mesh, nullptr, cot_scale, out, nullptr);
+        gather_kernel<3, G_GRAD, false><<<grid, env_threads("PM_GATHER_THREADS", 256), 0, c->stream>>>(map, g, c->rec, c->offsets, mesh, nullptr, cot_scale, out, nullptr);
     else if (C == 3)
-        gather_kernel<3, G_GRAD, true><<<grid, 256, 0, c->stream>>>(map, g, c->rec, c->offsets, mesh, cot, cot_scale, out, nullptr);
+        gather_kernel<3, G_GRAD, true><<<grid, env_threads("PM_GATHER_THREADS", 256), 0, c->stream>>>(map, g, c->rec, c->offsets, mesh, cot, cot_scale, out, nullptr);
     else
         return fail(c, PM_EINVAL, "gather_grad", "C must be 1 or 3");
     PM_LAUNCH_CHECK(c, "gather_kernel<grad>");
@@ -589,7 +618,7 @@ int gather_fused_sorted(pm_ctx *c, const float *mesh4, int zs, long long ms, con
     CicGeom g = make_cic_geom(c, mesh4, 4, zs, ms, false, &map);
     double np = (double)c->cur_np, ng = (double)c->g.ng;
     Timer t(c, TC_GATHER_FUSED, 48.0 * np + 16.0 * ng);
-    gather_kernel<4, G_FUSED, true><<<tile_grid(c->g), 256, 0, c->stream>>>(map, g, c->rec, c->offsets, mesh4, pi, 1.f, acc, alpha);
+    gather_kernel<4, G_FUSED, true><<<tile_grid(c->g), env_threads("PM_GATHER_THREADS", 256), 0, c->stream>>>(map, g, c->rec, c->offsets, mesh4, pi, 1.f, acc, alpha);
     PM_LAUNCH_CHECK(c, "gather_kernel<fused>");
     t.stop();
     return PM_OK;
