@@ -5,12 +5,12 @@
 #include <cstring>
 #include <new>
 
-#include "pm_internal.cuh"
+#include "pm_pos.cuh"
 
 namespace pm {
 
 const char *const kTimingNames[TC_NCLASSES] = {
-    "bin_count", "bin_scan", "bin_reorder", "scatter1", "scatter3", "gather", "gather_grad", "gather_fused",
+    "bin_count", "bin_scan", "bin_reorder", "scatter1", "scatter3", "gather", "gather_grad", "gather_fused", "gather_kick",
     "kspace_force", "kspace_adjoint", "fft_r2c", "fft_c2r", "kick_drift", "objective", "convert"};
 
 static thread_local std::string g_err_noctx;
@@ -82,9 +82,9 @@ static int make_geometry(const pm_params *p, Geometry *g, const char **why)
     for (int d = 0; d < 3; d++) {
         g->N[d] = p->mesh[d];
         g->L[d] = p->lattice[d];
-        unsigned long long M = (unsigned long long)g->N[d] << g->fbits;
-        if (M % (unsigned long long)g->L[d]) { *why = "(mesh[d] << fbits) must be divisible by lattice[d]"; return PM_EINVAL; }
-        g->qstep[d] = M / (unsigned long long)g->L[d];
+        long long M = (long long)g->N[d] << XBITS;
+        if (M % (long long)g->L[d]) { *why = "(mesh[d] << 32) must be divisible by lattice[d]"; return PM_EINVAL; }
+        g->qstep[d] = M / (long long)g->L[d];
         g->np *= g->L[d];
         g->ng *= g->N[d];
     }
@@ -124,8 +124,9 @@ static size_t carve_workspace(pm_ctx *c, const Geometry &g, void *base)
     uint4 *rec = w.take<uint4>((size_t)g.np);
     int *offsets = w.take<int>((size_t)g.nkeys + 1);
     int *cursor = w.take<int>((size_t)g.nkeys + 1);
-    int *blocksum = w.take<int>((size_t)(g.nkeys + 1) / 4096 + 2);
-    int *s = w.take<int>((size_t)g.np * 3);
+    int *hist = w.take<int>((size_t)g.nkeys + 1);
+    unsigned long long *scan_agg = w.take<unsigned long long>((size_t)(g.nkeys + 1) / 4096 + 2);
+    long long *x = w.take<long long>((size_t)g.np * 3);
     long long *p = w.take<long long>((size_t)g.np * 3);
     float *acc = w.take<float>((size_t)g.np * 3);
     float *xi = w.take<float>((size_t)g.np * 3);
@@ -134,12 +135,12 @@ static size_t carve_workspace(pm_ctx *c, const Geometry &g, void *base)
     double *scal = w.take<double>(4096);
     int tabn = g.N[0] > g.N[1] ? g.N[0] : g.N[1];
     if (g.N[2] > tabn) tabn = g.N[2];
-    float *ktab = w.take<float>((size_t)9 * tabn);
+    double *ktab = w.take<double>((size_t)9 * tabn);
     void *fftw = w.take<char>(fft_work_reserve(g));
     if (c) {
         for (int k = 0; k < 7; k++) c->mesh[k] = m + (size_t)k * g.mesh_stride;
-        c->rec = rec; c->offsets = offsets; c->cursor = cursor; c->blocksum = blocksum;
-        c->s = s; c->p = p; c->acc = acc; c->xi = xi; c->pi = pi; c->alpha = alpha;
+        c->rec = rec; c->offsets = offsets; c->cursor = cursor; c->hist = hist; c->scan_agg = scan_agg;
+        c->x = x; c->p = p; c->acc = acc; c->xi = xi; c->pi = pi; c->alpha = alpha;
         c->scal = scal; c->ktab = ktab; c->ktabn = tabn;
         c->fft_work = fftw; c->fft_work_bytes = fft_work_reserve(g);
     }
@@ -206,7 +207,7 @@ static int upload_ktab(pm_ctx *c)
 {
     const Geometry &g = c->g;
     int tn = c->ktabn;
-    std::vector<float> h((size_t)9 * tn, 0.f);
+    std::vector<double> h((size_t)9 * tn, 0.0);
     const double PI = 3.14159265358979323846264338327950288;
     for (int d = 0; d < 3; d++) {
         int N = g.N[d];
@@ -219,12 +220,12 @@ static int upload_ktab(pm_ctx *c)
                 double hh = 0.5 * k, sc = std::sin(hh) / hh;
                 dec = 1.0 / (sc * sc * sc * sc);
             }
-            h[(size_t)(3 * d + 0) * tn + i] = (float)(nyq ? 0.0 : k);
-            h[(size_t)(3 * d + 1) * tn + i] = (float)(k * k);
-            h[(size_t)(3 * d + 2) * tn + i] = (float)dec;
+            h[(size_t)(3 * d + 0) * tn + i] = nyq ? 0.0 : k;
+            h[(size_t)(3 * d + 1) * tn + i] = k * k;
+            h[(size_t)(3 * d + 2) * tn + i] = dec;
         }
     }
-    PM_CUDA(c, cudaMemcpy(c->ktab, h.data(), sizeof(float) * h.size(), cudaMemcpyHostToDevice));
+    PM_CUDA(c, cudaMemcpy(c->ktab, h.data(), sizeof(double) * h.size(), cudaMemcpyHostToDevice));
     return PM_OK;
 }
 
@@ -281,6 +282,7 @@ int pm_init(pm_ctx **out, const pm_params *params, void *dev_workspace, size_t b
     c->t_index = -1;
     c->have_adjoint = false;
     c->sorted_valid = false;
+    c->hist_valid = false;
     c->timing_on = false;
     c->n_own = c->n_fft = 0;
     c->cur_np = 0;
@@ -300,6 +302,11 @@ int pm_init(pm_ctx **out, const pm_params *params, void *dev_workspace, size_t b
     rc = make_plans(c);
     if (rc == PM_OK) rc = cic_init_tensor_maps(c);
     if (rc == PM_OK) rc = upload_ktab(c);
+    c->scan_epoch = 0;
+    if (rc == PM_OK && (cudaMemsetAsync(c->scan_agg, 0, sizeof(unsigned long long) * ((size_t)(g.nkeys + 1) / 4096 + 2), c->stream) != cudaSuccess ||
+                        cudaMemsetAsync(c->hist, 0, sizeof(int) * ((size_t)g.nkeys + 1), c->stream) != cudaSuccess ||
+                        cudaStreamSynchronize(c->stream) != cudaSuccess))
+        rc = fail(c, PM_ECUDA, "pm_init", "clearing the key histogram");
     if (rc != PM_OK) {
         g_err_noctx = c->err;
         pm_destroy(c);

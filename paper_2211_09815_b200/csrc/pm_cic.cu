@@ -22,7 +22,7 @@
 //   for the particles of its own tile; results go to out[j] in the caller's particle order.
 #include <cstdlib>
 
-#include "pm_internal.cuh"
+#include "pm_pos.cuh"
 
 namespace pm {
 
@@ -34,6 +34,9 @@ struct CicGeom {
     int use_tma;   // tensor map valid for this mesh
     int c0;        // first component (4th tensor-map coordinate)
     int kshift;    // debug: coarsen the scatter's fixed-point scale by this many bits (0 in production)
+    double mean;   // unit-mass scatter only: constant subtracted from every mesh point IN INTEGER, before the
+                   // int -> fp32 conversion (0 = plain density; nbar on the force path, whose k = 0 mode is zeroed
+                   // anyway, so that fp32 rounding is relative to the fluctuation rho - nbar, not to rho)
 };
 
 constexpr int TILE_PTS = TX * TY * TZ;
@@ -143,6 +146,7 @@ static CicGeom make_cic_geom(pm_ctx *c, const float *mesh, int C, int zs, long l
     r.use_tma = 0;
     r.c0 = 0;
     { const char *e = getenv("PM_DEBUG_KSHIFT"); r.kshift = e ? atoi(e) : 0; }
+    r.mean = 0.0;
     memset(map, 0, sizeof(*map));
     long long off = mesh - c->mesh[0];
     bool internal = zs == g.zs && ms == g.mesh_stride && mesh >= c->mesh[0] && off % g.mesh_stride == 0 &&
@@ -350,6 +354,14 @@ __global__ void __launch_bounds__(256) scatter_kernel(const __grid_constant__ CU
         scale = ldexpf(room / fmaxf(bound, 1.f), -g.kshift);
     }
     const float inv_scale = 1.f / scale;
+    // mean subtraction (unit mass): mq quanta are removed exactly in integer, the sub-quantum rest in fp32
+    long long mq = 0;
+    float mrest = 0.f;
+    if (!HAS_VAL && g.mean != 0.0) {
+        const double m = g.mean * (double)scale;
+        mq = __double2ll_rn(m);
+        mrest = (float)((m - (double)mq) * (double)inv_scale);
+    }
     const float fr = 1.f / (float)(1u << g.fbits);
     const unsigned fmask = (1u << g.fbits) - 1u;
 
@@ -375,8 +387,8 @@ __global__ void __launch_bounds__(256) scatter_kernel(const __grid_constant__ CU
         for (int i = threadIdx.x; i < C * TILE_PTS / 4; i += blockDim.x) {
             int4 a = a4[i];
             float4 f = HAS_VAL ? make_float4((float)a.x * inv_scale, (float)a.y * inv_scale, (float)a.z * inv_scale, (float)a.w * inv_scale)
-                               : make_float4((float)(unsigned)a.x * inv_scale, (float)(unsigned)a.y * inv_scale,
-                                             (float)(unsigned)a.z * inv_scale, (float)(unsigned)a.w * inv_scale);
+                               : make_float4((float)((long long)(unsigned)a.x - mq) * inv_scale - mrest, (float)((long long)(unsigned)a.y - mq) * inv_scale - mrest,
+                                             (float)((long long)(unsigned)a.z - mq) * inv_scale - mrest, (float)((long long)(unsigned)a.w - mq) * inv_scale - mrest);
             reinterpret_cast<float4 *>(a4)[i] = f;
         }
         fence_proxy_async_smem();
@@ -396,7 +408,7 @@ __global__ void __launch_bounds__(256) scatter_kernel(const __grid_constant__ CU
 #pragma unroll
                 for (int c = 0; c < C; c++) {
                     const int a = tile_acc[c][row * TZ + lane];
-                    mesh[(size_t)c * g.ms + o] = (HAS_VAL ? (float)a : (float)(unsigned)a) * inv_scale;
+                    mesh[(size_t)c * g.ms + o] = HAS_VAL ? (float)a * inv_scale : (float)((long long)(unsigned)a - mq) * inv_scale - mrest;
                 }
             }
         }
@@ -408,11 +420,16 @@ __global__ void __launch_bounds__(256) scatter_kernel(const __grid_constant__ CU
 // --------------------------------------------------------------------------------------------------
 enum GatherMode { G_VALUE = 0, G_GRAD = 1, G_FUSED = 2 };
 
-template <int C, int MODE, bool HAS_COT>
+// KICK: the interpolated acc (and alpha) of a particle is applied on the spot -- p += rn(acc Ka) [+= rn(acc Kb)],
+// x += rn(p D), and for the adjoint xi -= alpha K, pi -= xi D (eq. 16 L172 / eq. 49, same arithmetic and
+// order as kick_drift_kernel) -- and the particle's new sort key is added to the histogram of the next sort, so
+// a step needs no separate kick/drift and histogram passes and acc/alpha never travel through HBM.
+template <int C, int MODE, bool HAS_COT, bool KICK>
 __global__ void __launch_bounds__(256) gather_kernel(const __grid_constant__ CUtensorMap tmap, CicGeom g,
                                                      const uint4 *__restrict__ rec, const int *__restrict__ offsets,
-                                                     const float *__restrict__ mesh, const float *__restrict__ cot,
-                                                     float cot_scale, float *__restrict__ out, float *__restrict__ out2)
+                                                     const float *__restrict__ mesh, const float *cot,
+                                                     float cot_scale, float *__restrict__ out, float *__restrict__ out2,
+                                                     PosGeom pg, KickArgs ka)
 {
     __shared__ __align__(128) float halo[C * HALO_STRIDE];
     __shared__ __align__(8) unsigned long long bar;
@@ -466,6 +483,17 @@ __global__ void __launch_bounds__(256) gather_kernel(const __grid_constant__ CUt
     const unsigned fmask = (1u << g.fbits) - 1u;
     for (int i = beg + threadIdx.x; i < end; i += blockDim.x) {
         if (i != beg + (int)threadIdx.x) q = rec[i];
+        // KICK: the particle's state is fetched first (independent loads, in flight while the weights are formed)
+        long long st_p[3], st_x[3];
+        float st_xi[3];
+        if (KICK) {
+#pragma unroll
+            for (int d = 0; d < 3; d++) {
+                st_p[d] = ka.p[3 * (size_t)q.w + d];
+                if (ka.Ds != 0.0) st_x[d] = ka.x[3 * (size_t)q.w + d];
+                if (MODE == G_FUSED) st_xi[d] = ka.xi[3 * (size_t)q.w + d];
+            }
+        }
         const unsigned X[3] = {q.x, q.y, q.z};
         int l[3];
         float w[3][2];
@@ -516,7 +544,38 @@ __global__ void __launch_bounds__(256) gather_kernel(const __grid_constant__ CUt
                         gr[2] += dWz * m;
                     }
                 }
-        if (MODE == G_VALUE) {
+        if (KICK) {
+            const float *a3 = MODE == G_FUSED ? &val[1] : &val[0];
+            unsigned int Xn[3];
+#pragma unroll
+            for (int d = 0; d < 3; d++) {
+                const size_t i = 3 * j + d;
+                long long pv = st_p[d];
+                if (ka.Ka != 0.0) pv += __double2ll_rn((double)a3[d] * ka.Ka);
+                if (ka.Kb != 0.0) pv += __double2ll_rn((double)a3[d] * ka.Kb);
+                ka.p[i] = pv;
+                if (MODE == G_FUSED) {
+                    float v = st_xi[d];
+                    if (ka.Ka != 0.0) v = fmaf(-gr[d], ka.Kaf, v);
+                    if (ka.Kb != 0.0) v = fmaf(-gr[d], ka.Kbf, v);
+                    ka.xi[i] = v;
+                    if (ka.Ds != 0.0) ka.pi[i] = fmaf(-v, ka.Df, cv[1 + d]);
+                }
+                if (ka.Ds != 0.0) {
+                    const long long xv = st_x[d] + __double2ll_rn((double)pv * ka.Ds);
+                    ka.x[i] = xv;
+                    Xn[d] = record_coord(pg, xv, d);
+                }
+            }
+            if (ka.Ds != 0.0) hist_add(ka.hist, key_of(pg, Xn));
+            if (ka.store) {
+#pragma unroll
+                for (int e = 0; e < 3; e++) {
+                    out[j * 3 + e] = a3[e];
+                    if (MODE == G_FUSED) out2[j * 3 + e] = gr[e];
+                }
+            }
+        } else if (MODE == G_VALUE) {
 #pragma unroll
             for (int c = 0; c < C; c++) out[j * C + c] = val[c];
         } else if (MODE == G_GRAD) {
@@ -540,10 +599,11 @@ static int env_threads(const char *name, int dflt)
     return (v >= 32 && v <= 256 && v % 32 == 0) ? v : dflt;
 }
 
-int scatter_sorted(pm_ctx *c, const float *val, int C, float *mesh, int zs, long long ms)
+int scatter_sorted(pm_ctx *c, const float *val, int C, float *mesh, int zs, long long ms, double mean)
 {
     CUtensorMap map;
     CicGeom g = make_cic_geom(c, mesh, C, zs, ms, true, &map);
+    g.mean = (C == 1 && !val) ? mean : 0.0;
     double np = (double)c->cur_np, ng = (double)c->g.ng;
     dim3 grid = tile_grid(c->g);
     if (C == 1 && !val) {
@@ -567,21 +627,38 @@ int scatter_sorted(pm_ctx *c, const float *val, int C, float *mesh, int zs, long
     return PM_OK;
 }
 
-int gather_sorted(pm_ctx *c, const float *mesh, int C, int zs, long long ms, float *out)
+static double kick_bytes(const KickArgs *ka, bool adj)
+{
+    // per particle: p read + write, x read + write on a drift, xi read + write and pi write for the adjoint, stores
+    double b = 48.0 + (ka->Ds != 0.0 ? 48.0 : 0.0) + (ka->store ? (adj ? 24.0 : 12.0) : 0.0);
+    if (adj) b += 24.0 + (ka->Ds != 0.0 ? 12.0 : 0.0);
+    return b;
+}
+
+int gather_sorted(pm_ctx *c, const float *mesh, int C, int zs, long long ms, float *out, const KickArgs *ka)
 {
     CUtensorMap map;
     CicGeom g = make_cic_geom(c, mesh, C, zs, ms, false, &map);
     double np = (double)c->cur_np, ng = (double)c->g.ng;
     dim3 grid = tile_grid(c->g);
+    PosGeom pg = make_pos_geom(c->g);
+    KickArgs none;
+    memset(&none, 0, sizeof none);
+    if (ka && C != 3) return fail(c, PM_EINVAL, "gather", "internal: kick needs C = 3");
     if (C == 1) {
         Timer t(c, TC_GATHER3, 16.0 * np + 4.0 * ng);
-        gather_kernel<1, G_VALUE, false><<<grid, env_threads("PM_GATHER_THREADS", 256), 0, c->stream>>>(map, g, c->rec, c->offsets, mesh, nullptr, 1.f, out, nullptr);
+        gather_kernel<1, G_VALUE, false, false><<<grid, env_threads("PM_GATHER_THREADS", 256), 0, c->stream>>>(map, g, c->rec, c->offsets, mesh, nullptr, 1.f, out, nullptr, pg, none);
         PM_LAUNCH_CHECK(c, "gather_kernel<1>");
         t.stop();
-    } else if (C == 3) {
+    } else if (C == 3 && !ka) {
         Timer t(c, TC_GATHER3, 24.0 * np + 12.0 * ng);
-        gather_kernel<3, G_VALUE, false><<<grid, env_threads("PM_GATHER_THREADS", 256), 0, c->stream>>>(map, g, c->rec, c->offsets, mesh, nullptr, 1.f, out, nullptr);
+        gather_kernel<3, G_VALUE, false, false><<<grid, env_threads("PM_GATHER_THREADS", 256), 0, c->stream>>>(map, g, c->rec, c->offsets, mesh, nullptr, 1.f, out, nullptr, pg, none);
         PM_LAUNCH_CHECK(c, "gather_kernel<3>");
+        t.stop();
+    } else if (C == 3) {
+        Timer t(c, TC_GATHER_KICK, (12.0 + kick_bytes(ka, false)) * np + 12.0 * ng);
+        gather_kernel<3, G_VALUE, false, true><<<grid, env_threads("PM_GATHER_THREADS", 256), 0, c->stream>>>(map, g, c->rec, c->offsets, mesh, nullptr, 1.f, out, nullptr, pg, *ka);
+        PM_LAUNCH_CHECK(c, "gather_kernel<3,kick>");
         t.stop();
     } else {
         return fail(c, PM_EINVAL, "gather", "C must be 1 or 3");
@@ -596,15 +673,19 @@ int gather_grad_sorted(pm_ctx *c, const float *mesh, int C, int zs, long long ms
     CicGeom g = make_cic_geom(c, mesh, C, zs, ms, false, &map);
     double np = (double)c->cur_np, ng = (double)c->g.ng;
     dim3 grid = tile_grid(c->g);
+    PosGeom pg = make_pos_geom(c->g);
+    KickArgs none;
+    memset(&none, 0, sizeof none);
+    const int th = env_threads("PM_GATHER_THREADS", 256);
     Timer t(c, TC_GATHER_GRAD, (24.0 + (cot ? 4.0 * C : 0.0)) * np + 4.0 * C * ng);
     if (C == 1 && !cot)
-        gather_kernel<1, G_GRAD, false><<<grid, env_threads("PM_GATHER_THREADS", 256), 0, c->stream>>>(map, g, c->rec, c->offsets, mesh, nullptr, cot_scale, out, nullptr);
+        gather_kernel<1, G_GRAD, false, false><<<grid, th, 0, c->stream>>>(map, g, c->rec, c->offsets, mesh, nullptr, cot_scale, out, nullptr, pg, none);
     else if (C == 1)
-        gather_kernel<1, G_GRAD, true><<<grid, env_threads("PM_GATHER_THREADS", 256), 0, c->stream>>>(map, g, c->rec, c->offsets, mesh, cot, cot_scale, out, nullptr);
+        gather_kernel<1, G_GRAD, true, false><<<grid, th, 0, c->stream>>>(map, g, c->rec, c->offsets, mesh, cot, cot_scale, out, nullptr, pg, none);
     else if (C == 3 && !cot)
-        gather_kernel<3, G_GRAD, false><<<grid, env_threads("PM_GATHER_THREADS", 256), 0, c->stream>>>(map, g, c->rec, c->offsets, mesh, nullptr, cot_scale, out, nullptr);
+        gather_kernel<3, G_GRAD, false, false><<<grid, th, 0, c->stream>>>(map, g, c->rec, c->offsets, mesh, nullptr, cot_scale, out, nullptr, pg, none);
     else if (C == 3)
-        gather_kernel<3, G_GRAD, true><<<grid, env_threads("PM_GATHER_THREADS", 256), 0, c->stream>>>(map, g, c->rec, c->offsets, mesh, cot, cot_scale, out, nullptr);
+        gather_kernel<3, G_GRAD, true, false><<<grid, th, 0, c->stream>>>(map, g, c->rec, c->offsets, mesh, cot, cot_scale, out, nullptr, pg, none);
     else
         return fail(c, PM_EINVAL, "gather_grad", "C must be 1 or 3");
     PM_LAUNCH_CHECK(c, "gather_kernel<grad>");
@@ -612,15 +693,27 @@ int gather_grad_sorted(pm_ctx *c, const float *mesh, int C, int zs, long long ms
     return PM_OK;
 }
 
-int gather_fused_sorted(pm_ctx *c, const float *mesh4, int zs, long long ms, const float *pi, float *acc, float *alpha)
+int gather_fused_sorted(pm_ctx *c, const float *mesh4, int zs, long long ms, const float *pi, float *acc, float *alpha,
+                        const KickArgs *ka)
 {
     CUtensorMap map;
     CicGeom g = make_cic_geom(c, mesh4, 4, zs, ms, false, &map);
     double np = (double)c->cur_np, ng = (double)c->g.ng;
-    Timer t(c, TC_GATHER_FUSED, 48.0 * np + 16.0 * ng);
-    gather_kernel<4, G_FUSED, true><<<tile_grid(c->g), env_threads("PM_GATHER_THREADS", 256), 0, c->stream>>>(map, g, c->rec, c->offsets, mesh4, pi, 1.f, acc, alpha);
-    PM_LAUNCH_CHECK(c, "gather_kernel<fused>");
-    t.stop();
+    PosGeom pg = make_pos_geom(c->g);
+    const int th = env_threads("PM_GATHER_THREADS", 256);
+    if (!ka) {
+        KickArgs none;
+        memset(&none, 0, sizeof none);
+        Timer t(c, TC_GATHER_FUSED, 48.0 * np + 16.0 * ng);
+        gather_kernel<4, G_FUSED, true, false><<<tile_grid(c->g), th, 0, c->stream>>>(map, g, c->rec, c->offsets, mesh4, pi, 1.f, acc, alpha, pg, none);
+        PM_LAUNCH_CHECK(c, "gather_kernel<fused>");
+        t.stop();
+    } else {
+        Timer t(c, TC_GATHER_FUSED, (24.0 + kick_bytes(ka, true)) * np + 16.0 * ng);
+        gather_kernel<4, G_FUSED, true, true><<<tile_grid(c->g), th, 0, c->stream>>>(map, g, c->rec, c->offsets, mesh4, pi, 1.f, acc, alpha, pg, *ka);
+        PM_LAUNCH_CHECK(c, "gather_kernel<fused,kick>");
+        t.stop();
+    }
     return PM_OK;
 }
 

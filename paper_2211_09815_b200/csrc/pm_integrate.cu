@@ -2,11 +2,11 @@
 //
 // PAPER.md eq. 16 (L172): K: p += acc K;  D: x += p D;  eq. 49 (L393): the adjoint step undoes them in
 // reverse order with the time arguments swapped, D(tc,ta,tb) = -D(tc,tb,ta) (L389), and advances
-// xi -= alpha K, pi -= xi D alongside.  The state is held in fixed point (s: int32 * 2^-fbits cells,
+// xi -= alpha K, pi -= xi D alongside.  The state is held in fixed point (x = q + s: int64 * 2^-XBITS cells,
 // p: int64 * 2^-PBITS) so that "+= round(v)" followed by "+= round(-v)" restores it bit for bit: the
 // reverse pass then re-evaluates F at exactly the forward positions (
 // L371 names "more precise floating-point numbers" as the paper's remedy for fp32 irreversibility).
-#include "pm_internal.cuh"
+#include "pm_pos.cuh"
 
 namespace pm {
 
@@ -18,55 +18,83 @@ static inline int ew_blocks(long long n)
     return (int)b;
 }
 
-__global__ void __launch_bounds__(256) state_from_float_kernel(long long n3, const float *__restrict__ s, const float *__restrict__ p,
-                                                               double sscale, double pscale, int *__restrict__ sf,
-                                                               long long *__restrict__ pf)
+// lattice site of particle j in state units (q_j = (jx, jy, jz) * N/L cells, R6)
+__device__ __forceinline__ void lattice_site(const PosGeom &g, long long j, long long q[3])
+{
+    long long jz = j % g.L[2], t = j / g.L[2];
+    long long jy = t % g.L[1], jx = t / g.L[1];
+    q[0] = jx * g.qstep[0];
+    q[1] = jy * g.qstep[1];
+    q[2] = jz * g.qstep[2];
+}
+
+__global__ void __launch_bounds__(256) state_from_float_kernel(PosGeom g, long long np, const float *__restrict__ s,
+                                                               const float *__restrict__ p, double xscale, double pscale,
+                                                               long long *__restrict__ xf, long long *__restrict__ pf)
 {
     long long stride = (long long)gridDim.x * blockDim.x;
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n3; i += stride) {
-        sf[i] = (int)__double2ll_rn((double)s[i] * sscale);
-        pf[i] = __double2ll_rn((double)p[i] * pscale);
+    for (long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x; j < np; j += stride) {
+        long long q[3];
+        lattice_site(g, j, q);
+#pragma unroll
+        for (int d = 0; d < 3; d++) {
+            xf[3 * j + d] = q[d] + __double2ll_rn((double)s[3 * j + d] * xscale);
+            pf[3 * j + d] = __double2ll_rn((double)p[3 * j + d] * pscale);
+        }
     }
 }
 
-__global__ void __launch_bounds__(256) state_to_float_kernel(long long n3, const int *__restrict__ sf, const long long *__restrict__ pf,
-                                                             double inv_sscale, double inv_pscale, float *__restrict__ s,
-                                                             float *__restrict__ p)
+__global__ void __launch_bounds__(256) state_to_float_kernel(PosGeom g, long long np, const long long *__restrict__ xf,
+                                                             const long long *__restrict__ pf, double inv_xscale,
+                                                             double inv_pscale, float *__restrict__ s, float *__restrict__ p)
 {
     long long stride = (long long)gridDim.x * blockDim.x;
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n3; i += stride) {
-        if (s) s[i] = (float)((double)sf[i] * inv_sscale);
-        if (p) p[i] = (float)((double)pf[i] * inv_pscale);
+    for (long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x; j < np; j += stride) {
+        long long q[3];
+        lattice_site(g, j, q);
+#pragma unroll
+        for (int d = 0; d < 3; d++) {
+            if (s) s[3 * j + d] = (float)((double)(xf[3 * j + d] - q[d]) * inv_xscale);
+            if (p) p[3 * j + d] = (float)((double)pf[3 * j + d] * inv_pscale);
+        }
     }
 }
 
-// Ks = K * 2^PBITS, Ds = D * 2^fbits / 2^PBITS.  ADJ also advances xi, pi with the plain K, D.
+// Ks = K * 2^PBITS, Ds = D * 2^(XBITS - PBITS).  ADJ also advances xi, pi with the plain K, D.
+// One thread per particle; a drift also adds the particle's new sort key to the histogram of the next sort.
 template <bool ADJ>
-__global__ void __launch_bounds__(256) kick_drift_kernel(long long n3, double Ks, double Ds, float K, float D,
-                                                         int *__restrict__ s, long long *__restrict__ p,
+__global__ void __launch_bounds__(256) kick_drift_kernel(PosGeom g, long long np, double Ks, double Ds, float K, float D,
+                                                         long long *__restrict__ x, long long *__restrict__ p,
                                                          const float *__restrict__ acc, float *__restrict__ xi,
-                                                         float *__restrict__ pi, const float *__restrict__ alpha)
+                                                         float *__restrict__ pi, const float *__restrict__ alpha,
+                                                         int *__restrict__ hist)
 {
     long long stride = (long long)gridDim.x * blockDim.x;
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n3; i += stride) {
-        long long pv = p[i];
-        if (Ks != 0.0) {
-            pv += __double2ll_rn((double)acc[i] * Ks);
-            p[i] = pv;
-        }
-        if (Ds != 0.0) {
-            unsigned int sv = (unsigned int)s[i];
-            sv += (unsigned int)(int)__double2ll_rn((double)pv * Ds);  // wraps: displacement is periodic mod 2^(32-fbits) cells
-            s[i] = (int)sv;
-        }
-        if (ADJ) {
-            float x = xi[i];
+    for (long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x; j < np; j += stride) {
+        unsigned int X[3];
+#pragma unroll
+        for (int d = 0; d < 3; d++) {
+            const long long i = 3 * j + d;
+            long long pv = p[i];
             if (Ks != 0.0) {
-                x = fmaf(-alpha[i], K, x);
-                xi[i] = x;
+                pv += __double2ll_rn((double)acc[i] * Ks);
+                p[i] = pv;
             }
-            if (Ds != 0.0) pi[i] = fmaf(-x, D, pi[i]);
+            if (Ds != 0.0) {
+                long long xv = x[i] + __double2ll_rn((double)pv * Ds);
+                x[i] = xv;
+                X[d] = record_coord(g, xv, d);
+            }
+            if (ADJ) {
+                float v = xi[i];
+                if (Ks != 0.0) {
+                    v = fmaf(-alpha[i], K, v);
+                    xi[i] = v;
+                }
+                if (Ds != 0.0) pi[i] = fmaf(-v, D, pi[i]);
+            }
         }
+        if (Ds != 0.0) hist_add(hist, key_of(g, X));
     }
 }
 
@@ -116,9 +144,10 @@ __global__ void __launch_bounds__(256) combine_kernel(long long n3, const float 
 
 int state_from_float(pm_ctx *c, const float *s, const float *p)
 {
-    long long n3 = 3 * c->g.np;
-    Timer t(c, TC_CONVERT, 20.0 * n3);
-    state_from_float_kernel<<<ew_blocks(n3), 256, 0, c->stream>>>(n3, s, p, ldexp(1.0, c->g.fbits), ldexp(1.0, PBITS), c->s, c->p);
+    long long np = c->g.np;
+    Timer t(c, TC_CONVERT, 72.0 * np);
+    state_from_float_kernel<<<ew_blocks(np), 256, 0, c->stream>>>(make_pos_geom(c->g), np, s, p, ldexp(1.0, XBITS),
+                                                                  ldexp(1.0, PBITS), c->x, c->p);
     PM_LAUNCH_CHECK(c, "state_from_float_kernel");
     t.stop();
     return PM_OK;
@@ -126,37 +155,49 @@ int state_from_float(pm_ctx *c, const float *s, const float *p)
 
 int state_to_float(pm_ctx *c, float *s, float *p)
 {
-    long long n3 = 3 * c->g.np;
-    Timer t(c, TC_CONVERT, 20.0 * n3);
-    state_to_float_kernel<<<ew_blocks(n3), 256, 0, c->stream>>>(n3, c->s, c->p, ldexp(1.0, -c->g.fbits), ldexp(1.0, -PBITS), s, p);
+    long long np = c->g.np;
+    Timer t(c, TC_CONVERT, 72.0 * np);
+    state_to_float_kernel<<<ew_blocks(np), 256, 0, c->stream>>>(make_pos_geom(c->g), np, c->x, c->p, ldexp(1.0, -XBITS),
+                                                                ldexp(1.0, -PBITS), s, p);
     PM_LAUNCH_CHECK(c, "state_to_float_kernel");
     t.stop();
     return PM_OK;
 }
 
+// a drift invalidates the sort and leaves the key histogram of the new positions in c->hist
+static int drift_bookkeeping(pm_ctx *c, double D)
+{
+    if (D != 0.0) {
+        if (c->hist_valid) return fail(c, PM_ESTATE, "kick_drift", "internal: key histogram already pending");
+        c->sorted_valid = false;
+        c->hist_valid = true;
+    }
+    return PM_OK;
+}
+
 int kick_drift(pm_ctx *c, double K, double D)
 {
-    long long n3 = 3 * c->g.np;
-    double Ks = ldexp(K, PBITS), Ds = ldexp(D, c->g.fbits - PBITS);
-    Timer t(c, TC_KICK_DRIFT, (K != 0.0 ? 20.0 : 8.0) * n3 + (D != 0.0 ? 8.0 * n3 : 0.0));
-    kick_drift_kernel<false><<<ew_blocks(n3), 256, 0, c->stream>>>(n3, Ks, Ds, (float)K, (float)D, c->s, c->p, c->acc, nullptr,
-                                                                   nullptr, nullptr);
+    long long np = c->g.np;
+    double Ks = ldexp(K, PBITS), Ds = ldexp(D, XBITS - PBITS);
+    PM_TRY(drift_bookkeeping(c, D));
+    Timer t(c, TC_KICK_DRIFT, 3.0 * np * ((K != 0.0 ? 20.0 : 8.0) + (D != 0.0 ? 16.0 : 0.0)));
+    kick_drift_kernel<false><<<ew_blocks(np), 256, 0, c->stream>>>(make_pos_geom(c->g), np, Ks, Ds, (float)K, (float)D, c->x, c->p,
+                                                                   c->acc, nullptr, nullptr, nullptr, c->hist);
     PM_LAUNCH_CHECK(c, "kick_drift_kernel");
     t.stop();
-    if (D != 0.0) c->sorted_valid = false;
     return PM_OK;
 }
 
 int kick_drift_adj(pm_ctx *c, double K, double D)
 {
-    long long n3 = 3 * c->g.np;
-    double Ks = ldexp(K, PBITS), Ds = ldexp(D, c->g.fbits - PBITS);
-    Timer t(c, TC_KICK_DRIFT, (K != 0.0 ? 32.0 : 12.0) * n3 + (D != 0.0 ? 16.0 * n3 : 0.0));
-    kick_drift_kernel<true><<<ew_blocks(n3), 256, 0, c->stream>>>(n3, Ks, Ds, (float)K, (float)D, c->s, c->p, c->acc, c->xi,
-                                                                  c->pi, c->alpha);
+    long long np = c->g.np;
+    double Ks = ldexp(K, PBITS), Ds = ldexp(D, XBITS - PBITS);
+    PM_TRY(drift_bookkeeping(c, D));
+    Timer t(c, TC_KICK_DRIFT, 3.0 * np * ((K != 0.0 ? 32.0 : 12.0) + (D != 0.0 ? 24.0 : 0.0)));
+    kick_drift_kernel<true><<<ew_blocks(np), 256, 0, c->stream>>>(make_pos_geom(c->g), np, Ks, Ds, (float)K, (float)D, c->x, c->p,
+                                                                  c->acc, c->xi, c->pi, c->alpha, c->hist);
     PM_LAUNCH_CHECK(c, "kick_drift_kernel<adj>");
     t.stop();
-    if (D != 0.0) c->sorted_valid = false;
     return PM_OK;
 }
 

@@ -19,6 +19,7 @@ namespace pm {
 constexpr int TX = 8, TY = 8, TZ = 32;
 constexpr int NCLS = 8;
 constexpr int PBITS = 36;  // momentum fixed point: p_fix = p * 2^PBITS (int64)
+constexpr int XBITS = 32;  // position fixed point: x_fix = (q + s) * 2^XBITS (int64, absolute, not wrapped)
 
 // ---- timing classes ---------------------------------------------------------------------------------
 enum TimingClass {
@@ -30,6 +31,7 @@ enum TimingClass {
     TC_GATHER3,
     TC_GATHER_GRAD,
     TC_GATHER_FUSED,
+    TC_GATHER_KICK,
     TC_KSPACE_FORCE,
     TC_KSPACE_ADJ,
     TC_FFT_R2C,
@@ -60,7 +62,7 @@ struct Geometry {
     long long nk;    // complex modes Nx*Ny*(Nz/2+1)
     int ntiles;      // nt[0]*nt[1]*nt[2]
     int nkeys;       // ntiles * NCLS
-    unsigned long long qstep[3];  // lattice spacing in fixed point: (N << fbits) / L
+    long long qstep[3];  // lattice spacing in state units: (N << XBITS) / L
 };
 
 }  // namespace pm
@@ -78,13 +80,15 @@ struct pm_ctx {
     float *mesh[7];              // padded in-place R2C layout, contiguous
     uint4 *rec;                  // sorted records {X, Y, Z, j}
     int *offsets;                // nkeys + 1 exclusive prefix of the key histogram
-    int *cursor;                 // nkeys + 1 scratch (histogram, then running cursors)
-    int *blocksum;               // scan scratch
-    int *s;                      // [np][3] int32 displacement * 2^fbits
+    int *cursor;                 // nkeys + 1 running cursors of the reorder pass
+    int *hist;                   // nkeys + 1 key histogram; zero between sorts (the scan clears it)
+    unsigned long long *scan_agg;  // scan scratch: per-block totals tagged with the launch epoch
+    unsigned int scan_epoch;
+    long long *x;                // [np][3] int64 absolute position (q + s) * 2^XBITS, not wrapped
     long long *p;                // [np][3] int64 momentum * 2^PBITS
     float *acc, *xi, *pi, *alpha;  // [np][3]
     double *scal;                // device scalars: [0] = J
-    float *ktab;                 // [3 axes][3: kt, k^2, dec][ktabn] per-axis k-space tables
+    double *ktab;                // [3 axes][3: kt, k^2, dec][ktabn] per-axis k-space tables (fp64)
     int ktabn;
     long long cur_np;            // particles in the current sort
     CUtensorMap tmap_load, tmap_store;  // 4-D {z, y, x, mesh 0..6} views of the internal meshes: halo box / tile box
@@ -95,6 +99,7 @@ struct pm_ctx {
     int t_index;                 // state is at t_{t_index}; -1 = no state
     bool have_adjoint;
     bool sorted_valid;           // rec/offsets describe the current state's positions
+    bool hist_valid;             // hist holds the key histogram of the current state's positions
     // instrumentation
     bool timing_on;
     std::vector<pm::TimingRec> trecs;
@@ -138,8 +143,10 @@ double drift_factor_host(double om, double ac, double aa, double ab);
 double kick_factor_host(double om, double ac, double aa, double ab);
 
 // ---- binning (pm_bin.cu) ----------------------------------------------------------------------------
-// sort np particles given as absolute float positions (x != NULL) or as the ctx state s (x == NULL)
-int bin_particles(pm_ctx *c, long long np, const float *x);
+// particles given as absolute float positions (x != NULL) or as the ctx state (x == NULL):
+// bin_count adds their keys to c->hist (zero on entry); bin_sort scans c->hist (and clears it) and writes the records
+int bin_count(pm_ctx *c, long long np, const float *x);
+int bin_sort(pm_ctx *c, long long np, const float *x);
 
 // ---- CIC (pm_cic.cu): operate on the sorted records of the last bin_particles -----------------------
 // encode the two internal tensor maps (call once from pm_init); failure leaves tma_ok = false (plain loads)
@@ -147,13 +154,16 @@ int cic_init_tensor_maps(pm_ctx *c);
 // val: [np][C] in ORIGINAL particle order or NULL.  mesh: C meshes, row stride zs, mesh stride ms.
 // Internal meshes (pointers inside c->mesh[]) use the ctx's tensor maps; other pointers get a map encoded per call
 // when their layout allows TMA (16-byte aligned base and strides), else the kernels' plain load/store path.
-int scatter_sorted(pm_ctx *c, const float *val, int C, float *mesh, int zs, long long ms);
-int gather_sorted(pm_ctx *c, const float *mesh, int C, int zs, long long ms, float *out);
+// mean (unit-mass scatter only): constant removed from every mesh point before the conversion to fp32
+int scatter_sorted(pm_ctx *c, const float *val, int C, float *mesh, int zs, long long ms, double mean = 0.0);
+struct KickArgs;  // pm_pos.cuh
+// ka != NULL (C = 3): fused kick / kick / drift + key histogram on the interpolated acc (see gather_kernel)
+int gather_sorted(pm_ctx *c, const float *mesh, int C, int zs, long long ms, float *out, const KickArgs *ka = nullptr);
 int gather_grad_sorted(pm_ctx *c, const float *mesh, int C, int zs, long long ms, const float *cot,
                        float cot_scale, float *out);
 // acc_j = sum_g W f_d ; alpha_j = sum_g dW (psi + sum_d pi_d f_d); meshes: psi = mesh4[0], f = mesh4[1..3]
 int gather_fused_sorted(pm_ctx *c, const float *mesh4, int zs, long long ms, const float *pi, float *acc,
-                        float *alpha);
+                        float *alpha, const KickArgs *ka = nullptr);
 
 // ---- k-space (pm_kspace.cu) -------------------------------------------------------------------------
 int kspace_force(pm_ctx *c, const float2 *rho_k, float2 *f_k /*3 meshes, stride ms/2*/, double nbar);

@@ -17,25 +17,25 @@ struct KGeom {
     int zsc;            // complex elements per (padded) z-row in memory: zs / 2
     long long nk;       // complex elements per mesh
     long long cstride;  // complex elements between components (padded mesh stride / 2)
-    const float *tab;   // [3 axes][3: kt, k2, dec][tabn]
-    int tabn;
-    float c0;           // 3/2 Om / (nbar N_g)
+    const double *tab;  // [3 axes][3: kt, k2, dec][tabn], fp64: G(k) kt_d is rounded to fp32 ONCE, so the same
+    int tabn;           //   (coherent) relative error is not applied to a mode at every step
+    double c0;          // 3/2 Om / (nbar N_g)
 };
 
 // idx enumerates the Nx*Ny*(Nz/2+1) modes; returns the element offset of that mode in the padded mesh
-__device__ __forceinline__ size_t k_factors(const KGeom &g, long long idx, float kt[3], float *G)
+__device__ __forceinline__ size_t k_factors(const KGeom &g, long long idx, double kt[3], double *G)
 {
     int iz = (int)(idx % g.nzc);
     long long row = idx / g.nzc;
     int iy = (int)(row % g.N[1]);
     int ix = (int)(row / g.N[1]);
-    const float *tx = g.tab, *ty = g.tab + 3 * g.tabn, *tz = g.tab + 6 * g.tabn;
+    const double *tx = g.tab, *ty = g.tab + 3 * g.tabn, *tz = g.tab + 6 * g.tabn;
     kt[0] = tx[ix];
     kt[1] = ty[iy];
     kt[2] = tz[iz];
-    float k2 = tx[g.tabn + ix] + ty[g.tabn + iy] + tz[g.tabn + iz];
-    float dec = tx[2 * g.tabn + ix] * ty[2 * g.tabn + iy] * tz[2 * g.tabn + iz];
-    *G = (ix | iy | iz) == 0 ? 0.f : g.c0 * dec / k2;
+    double k2 = tx[g.tabn + ix] + ty[g.tabn + iy] + tz[g.tabn + iz];
+    double dec = tx[2 * g.tabn + ix] * ty[2 * g.tabn + iy] * tz[2 * g.tabn + iz];
+    *G = (ix | iy | iz) == 0 ? 0.0 : g.c0 * dec / k2;
     return (size_t)row * g.zsc + iz;
 }
 
@@ -43,12 +43,12 @@ __global__ void __launch_bounds__(256) kspace_force_kernel(KGeom g, const float2
 {
     long long stride = (long long)gridDim.x * blockDim.x;
     for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < g.nk; idx += stride) {
-        float kt[3], G;
+        double kt[3], G;
         size_t o = k_factors(g, idx, kt, &G);
         float2 r = rho_k[o];
 #pragma unroll
         for (int d = 0; d < 3; d++) {
-            float c = kt[d] * G;  // times +i: (re, im) -> (-c im, c re)
+            float c = (float)(kt[d] * G);  // times +i: (re, im) -> (-c im, c re)
             f_k[(size_t)d * g.cstride + o] = make_float2(-c * r.y, c * r.x);
         }
     }
@@ -58,17 +58,18 @@ __global__ void __launch_bounds__(256) kspace_adjoint_kernel(KGeom g, const floa
 {
     long long stride = (long long)gridDim.x * blockDim.x;
     for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < g.nk; idx += stride) {
-        float kt[3], G;
+        double kt[3], G;
         size_t o = k_factors(g, idx, kt, &G);
         float re = 0.f, im = 0.f;
 #pragma unroll
         for (int d = 0; d < 3; d++) {
             float2 v = Pi_k[(size_t)d * g.cstride + o];
-            re += kt[d] * v.x;
-            im += kt[d] * v.y;
+            float c = (float)(kt[d] * G);  // the same fp32 factors as the force kernel: exact transpose
+            re += c * v.x;
+            im += c * v.y;
         }
-        // times -i G: (re, im) -> (G im, -G re)
-        psi_k[o] = make_float2(G * im, -G * re);
+        // times -i: (re, im) -> (im, -re)
+        psi_k[o] = make_float2(im, -re);
     }
 }
 
@@ -82,7 +83,7 @@ static KGeom make_kgeom(pm_ctx *c, double nbar)
     k.cstride = c->g.mesh_stride / 2;
     k.tab = c->ktab;
     k.tabn = c->ktabn;
-    k.c0 = (float)(1.5 * c->prm.omega_m / (nbar * (double)c->g.ng));
+    k.c0 = 1.5 * c->prm.omega_m / (nbar * (double)c->g.ng);
     return k;
 }
 

@@ -203,7 +203,7 @@ def test_config0_forward_adjoint_parity(pmlib, orc):
         e = rel_l2(out[k].cpu().numpy(), ref[k])
         assert e <= 1e-3, f"{k} rel L2 {e}"
     # exact reversibility: the reverse pass returns the (fixed-point quantised) initial state bit for bit
-    fb = 22
+    fb = 32  # XBITS of the fixed-point position state
     s_q = np.rint(s0.astype(np.float64) * 2 ** fb) / 2 ** fb
     p_q = np.rint(p0.astype(np.float64) * 2.0 ** 36) / 2.0 ** 36
     assert np.array_equal(out["s_rec"].cpu().numpy(), s_q.astype(np.float32))
