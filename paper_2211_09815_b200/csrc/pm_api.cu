@@ -125,6 +125,7 @@ static size_t carve_workspace(pm_ctx *c, const Geometry &g, void *base)
     int *offsets = w.take<int>((size_t)g.nkeys + 1);
     int *cursor = w.take<int>((size_t)g.nkeys + 1);
     int *hist = w.take<int>((size_t)g.nkeys + 1);
+    int *sched = w.take<int>(64);
     unsigned long long *scan_agg = w.take<unsigned long long>((size_t)(g.nkeys + 1) / 4096 + 2);
     long long *x = w.take<long long>((size_t)g.np * 3);
     long long *p = w.take<long long>((size_t)g.np * 3);
@@ -139,7 +140,7 @@ static size_t carve_workspace(pm_ctx *c, const Geometry &g, void *base)
     void *fftw = w.take<char>(fft_work_reserve(g));
     if (c) {
         for (int k = 0; k < 7; k++) c->mesh[k] = m + (size_t)k * g.mesh_stride;
-        c->rec = rec; c->offsets = offsets; c->cursor = cursor; c->hist = hist; c->scan_agg = scan_agg;
+        c->rec = rec; c->offsets = offsets; c->cursor = cursor; c->hist = hist; c->sched = sched; c->scan_agg = scan_agg;
         c->x = x; c->p = p; c->acc = acc; c->xi = xi; c->pi = pi; c->alpha = alpha;
         c->scal = scal; c->ktab = ktab; c->ktabn = tabn;
         c->fft_work = fftw; c->fft_work_bytes = fft_work_reserve(g);
@@ -303,6 +304,12 @@ int pm_init(pm_ctx **out, const pm_params *params, void *dev_workspace, size_t b
     if (rc == PM_OK) rc = cic_init_tensor_maps(c);
     if (rc == PM_OK) rc = upload_ktab(c);
     c->scan_epoch = 0;
+    {
+        int dev = 0;
+        c->num_sms = 148;
+        if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, dev);
+    }
+    if (rc == PM_OK && cudaMemsetAsync(c->sched, 0, 64 * sizeof(int), c->stream) != cudaSuccess) rc = fail(c, PM_ECUDA, "pm_init", "clearing the tile scheduler");
     if (rc == PM_OK && (cudaMemsetAsync(c->scan_agg, 0, sizeof(unsigned long long) * ((size_t)(g.nkeys + 1) / 4096 + 2), c->stream) != cudaSuccess ||
                         cudaMemsetAsync(c->hist, 0, sizeof(int) * ((size_t)g.nkeys + 1), c->stream) != cudaSuccess ||
                         cudaStreamSynchronize(c->stream) != cudaSuccess))

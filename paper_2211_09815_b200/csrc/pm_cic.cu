@@ -6,21 +6,28 @@
 // Cell i_d = floor(x_d), t_d = x_d - i_d in [0,1): weight (1 - t_d) at i_d, t_d at i_d + 1 (periodic),
 // derivative -1 / +1 (floor convention, right derivative; R7).
 //
-// Input: the records sorted by (tile, class) of pm_bin.cu.  One CTA per mesh tile of TX x TY x TZ cells,
-// grid = (tiles_z, tiles_y, tiles_x).
+// Input: the records sorted by (tile, class) of pm_bin.cu; a tile is TX x TY x TZ cells.
 //
-// scatter -- OUTPUT-STATIONARY: the CTA owns the mesh points of its tile, pulls the particles of its
-//   own tile plus the last-cell-layer classes of its (up to 7) low-side neighbour tiles, accumulates in
-//   shared memory with NATIVE int32 atomics (fp32 shared atomics are CAS loops on sm_100a) in fixed
-//   point with a per-tile power-of-two scale chosen from sum|v| so that it cannot overflow, converts in
-//   place and writes the tile with ONE TMA tensor store (cp.async.bulk.tensor, clipped at the mesh edge):
-//   no zero-fill pass, no global atomics, every mesh point written exactly once, and a result that does
-//   not depend on the order in which particles arrive (bit-reproducible).
-// gather -- the halo box (TX+1)(TY+1)(TZ+4) of each mesh is brought into shared memory by TMA tensor
-//   loads signalled on an mbarrier (tiles touching the upper mesh edge, whose halo wraps periodically,
-//   and meshes whose layout TMA cannot address use plain coalesced row loads); the CTA then interpolates
-//   for the particles of its own tile; results go to out[j] in the caller's particle order.
+// Both kernels are PERSISTENT and WARP-SPECIALISED: a few CTAs per SM, each with one producer warp and
+// NCW consumer warps that talk through a ring of NST shared-memory stages guarded by full / empty
+// mbarriers.  The producer draws the next non-empty tile from a global counter (dense tiles do not stall
+// a static schedule), looks up its record runs, and starts the asynchronous copies of everything the
+// tile needs -- records by 1-D bulk copies, mesh halos by one TMA tensor load per mesh (tiles whose halo
+// wraps around the periodic edge: one bulk copy per halo row) -- all signalled on the stage's full
+// barrier, so the copies of tile n + 1 fly while the consumers work on tile n.
+//
+// scatter -- OUTPUT-STATIONARY: the CTA owns the mesh points of the tile, takes the particles of the
+//   tile itself plus the last-cell-layer classes of its (up to 7) low-side neighbour tiles, accumulates in
+//   shared memory with NATIVE int32 atomics (fp32 and 64-bit shared atomics are CAS loops on sm_100a)
+//   in fixed point with a per-tile scale that cannot overflow, converts in place and writes the tile
+//   with ONE asynchronous TMA tensor store per mesh (clipped at the mesh edge) from a double-buffered
+//   accumulator: no zero-fill pass, no global atomics, every mesh point written exactly once, and a
+//   result that does not depend on the order in which particles arrive (bit-reproducible).
+// gather -- the halo box (TX+1)(TY+1)(TZ+4) of each mesh sits in shared memory; the consumers
+//   interpolate values / weight gradients / both for the particles of the tile and, in the KICK variants,
+//   apply the kick(s) and the drift to the particle's fixed-point state on the spot (pm_pos.cuh).
 #include <cstdlib>
+#include <cstring>
 
 #include "pm_pos.cuh"
 
@@ -31,19 +38,28 @@ struct CicGeom {
     int fbits;
     int zs;        // floats per z-row
     long long ms;  // floats per mesh (component stride)
-    int use_tma;   // tensor map valid for this mesh
+    int use_tma;   // tensor map valid for this mesh (16-byte aligned base and strides)
     int c0;        // first component (4th tensor-map coordinate)
+    int dbg;       // debug bits (PM_DEBUG_CIC): 1 = gather skips the particle loop, 2 = gather skips the halo copies
+    int tma_halo;  // debug: 1 = interior halos by TMA tensor loads instead of 16-byte async copies (PM_DEBUG_TMA_HALO)
     int kshift;    // debug: coarsen the scatter's fixed-point scale by this many bits (0 in production)
+    int ntiles;
     double mean;   // unit-mass scatter only: constant subtracted from every mesh point IN INTEGER, before the
                    // int -> fp32 conversion (0 = plain density; nbar on the force path, whose k = 0 mode is zeroed
                    // anyway, so that fp32 rounding is relative to the fluctuation rho - nbar, not to rho)
+    int *sched;    // [0] tile counter, [1] finished CTAs; both zero between launches (the last CTA resets them)
 };
 
 constexpr int TILE_PTS = TX * TY * TZ;
-constexpr int HX = TX + 1, HY = TY + 1, HZ = TZ + 1;
+constexpr int HX = TX + 1, HY = TY + 1;
 constexpr int HZP = TZ + 4;                               // halo row pitch: 144 bytes, a TMA-legal box width
 constexpr int HALO_PTS = HX * HY * HZP;
 constexpr int HALO_STRIDE = (HALO_PTS + 31) / 32 * 32;    // per-mesh stride in shared memory: 128-byte multiple
+constexpr int NCW = 8;                                    // consumer warps
+constexpr int NCT = NCW * 32;                             // consumer threads
+constexpr int NTHREADS = NCT + 32;                        // + one producer warp
+constexpr int NST = 2;                                    // pipeline stages
+constexpr int RCAP = 512;                                 // records staged in shared memory per tile (the rest are read from global)
 
 // ---- PTX wrappers: mbarrier + TMA (sm_90+/sm_100a) ----------------------------------------------------
 __device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
@@ -51,22 +67,37 @@ __device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)_
 __device__ __forceinline__ void mbar_init(unsigned long long *bar, int count)
 {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
 }
+__device__ __forceinline__ void mbar_fence_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 __device__ __forceinline__ void mbar_expect_tx(unsigned long long *bar, unsigned bytes)
 {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
 }
+// expect-tx WITHOUT arriving (the thread arrives separately)
+__device__ __forceinline__ void mbar_expect_tx_only(unsigned long long *bar, unsigned bytes)
+{
+    asm volatile("mbarrier.expect_tx.relaxed.cta.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+// 16-byte asynchronous copy through the LSU path (no per-operation TMA cost: used for short / ragged pieces)
+__device__ __forceinline__ void cp_async16(void *dst, const void *src)
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst)), "l"((unsigned long long)src) : "memory");
+}
+// arrive on the barrier once all cp.async issued so far by this thread have landed (counts as this thread's arrival)
+__device__ __forceinline__ void cp_async_arrive(unsigned long long *bar)
+{
+    asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(unsigned long long *bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
 __device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned phase)
 {
-    unsigned ok = 0;
-    while (!ok) {
-        asm volatile(
-            "{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
-            : "=r"(ok)
-            : "r"(smem_u32(bar)), "r"(phase)
-            : "memory");
-    }
+    asm volatile(
+        "{\n .reg .pred p;\n WAIT_%=:\n mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n @p bra DONE_%=;\n bra WAIT_%=;\n DONE_%=:\n}"
+        ::"r"(smem_u32(bar)), "r"(phase)
+        : "memory");
 }
 __device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *m, unsigned long long *bar, int z, int y, int x, int c)
 {
@@ -75,18 +106,24 @@ __device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *m, uns
         ::"r"(smem_u32(dst)), "l"((unsigned long long)m), "r"(smem_u32(bar)), "r"(z), "r"(y), "r"(x), "r"(c)
         : "memory");
 }
+__device__ __forceinline__ void bulk_load(void *dst, const void *src, unsigned bytes, unsigned long long *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst)), "l"((unsigned long long)src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
 __device__ __forceinline__ void tma_store_4d(const CUtensorMap *m, const void *src, int z, int y, int x, int c)
 {
     asm volatile("cp.async.bulk.tensor.4d.global.shared::cta.bulk_group [%0, {%2, %3, %4, %5}], [%1];"
                  ::"l"((unsigned long long)m), "r"(smem_u32(src)), "r"(z), "r"(y), "r"(x), "r"(c)
                  : "memory");
 }
-__device__ __forceinline__ void tma_store_commit_and_wait()
-{
-    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-    asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
-}
+__device__ __forceinline__ void tma_store_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void tma_store_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void tma_store_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+// barrier among the consumer warps only (the producer warp never joins it)
+__device__ __forceinline__ void consumer_sync() { asm volatile("bar.sync 1, %0;" ::"n"(NCT) : "memory"); }
 
 // ---- host: tensor maps ------------------------------------------------------------------------------------
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
@@ -147,6 +184,10 @@ static CicGeom make_cic_geom(pm_ctx *c, const float *mesh, int C, int zs, long l
     r.c0 = 0;
     { const char *e = getenv("PM_DEBUG_KSHIFT"); r.kshift = e ? atoi(e) : 0; }
     r.mean = 0.0;
+    r.ntiles = g.ntiles;
+    { const char *e = getenv("PM_DEBUG_TMA_HALO"); r.tma_halo = e ? atoi(e) : 0; }
+    { const char *e = getenv("PM_DEBUG_CIC"); r.dbg = e ? atoi(e) : 0; }
+    r.sched = c->sched;
     memset(map, 0, sizeof(*map));
     long long off = mesh - c->mesh[0];
     bool internal = zs == g.zs && ms == g.mesh_stride && mesh >= c->mesh[0] && off % g.mesh_stride == 0 &&
@@ -162,27 +203,124 @@ static CicGeom make_cic_geom(pm_ctx *c, const float *mesh, int C, int zs, long l
     return r;
 }
 
-__device__ __forceinline__ void tile_coords(const CicGeom &g, int t[3], int t0[3], int ext[3])
+// ---- tiles and scheduling -----------------------------------------------------------------------------
+__device__ __forceinline__ void tile_coords(const CicGeom &g, int tile, int t[3], int t0[3], int ext[3])
 {
-    t[0] = blockIdx.z; t[1] = blockIdx.y; t[2] = blockIdx.x;
+    t[2] = tile % g.nt[2];
+    const int r = tile / g.nt[2];
+    t[1] = r % g.nt[1];
+    t[0] = r / g.nt[1];
     t0[0] = t[0] * TX; t0[1] = t[1] * TY; t0[2] = t[2] * TZ;
     ext[0] = min(TX, g.N[0] - t0[0]);
     ext[1] = min(TY, g.N[1] - t0[1]);
     ext[2] = min(TZ, g.N[2] - t0[2]);
 }
 
-__device__ __forceinline__ float block_sum(float v, float *sh /*>= 32 floats*/)
+// Tiles are drawn from the global counter TBATCH at a time (neighbouring tiles share halo lines in L2, and the
+// atomic's round trip is paid once per batch); the next batch is requested one batch ahead.
+constexpr int TBATCH = 1;
+struct TileDraw {
+    int base, next_base, pos;
+    __device__ __forceinline__ void init(int *sched)
+    {
+        base = atomicAdd(&sched[0], TBATCH);
+        next_base = atomicAdd(&sched[0], TBATCH);
+        pos = 0;
+    }
+    // next tile index (may be >= ntiles: the caller stops there); uniform across the warp (lane 0 draws)
+    __device__ __forceinline__ int next(int *sched)
+    {
+        if (pos == TBATCH) {
+            base = next_base;
+            next_base = atomicAdd(&sched[0], TBATCH);
+            pos = 0;
+        }
+        return base + pos++;
+    }
+};
+
+// called by one thread per CTA when it has drawn its last tile: the last CTA to finish re-arms the counters
+__device__ __forceinline__ void sched_finish(int *sched)
 {
-    int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+    __threadfence();
+    if (atomicAdd(&sched[1], 1) == (int)gridDim.x - 1) {
+        sched[0] = 0;
+        sched[1] = 0;
+        __threadfence();
+    }
+}
+
+// CIC corners of one particle relative to a tile: local indices, ownership flags, weights.
+// FAST: the particle is of the tile's own class 0 (no coordinate in the last cell layer): all 8 corners are inside.
+template <bool FAST>
+struct Corners {
+    int l[3][2];
+    bool ok[3][2];
+    float w[3][2];
+    __device__ __forceinline__ Corners(const CicGeom &g, const int t0[3], const int ext[3], uint4 q, float fr, unsigned fmask)
+    {
+        const unsigned X[3] = {q.x, q.y, q.z};
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    if (lane == 0) sh[w] = v;
-    __syncthreads();
-    float r = 0.f;
-    for (int k = 0; k < nw; k++) r += sh[k];  // same order in every thread
-    __syncthreads();
+        for (int d = 0; d < 3; d++) {
+            int l0 = (int)(X[d] >> g.fbits) - t0[d];
+            int l1 = l0 + 1;
+            if (!FAST) {
+                if (l0 < 0) l0 += g.N[d];          // particle of the low neighbour across the periodic edge
+                l1 = l0 + 1;
+                if (l1 == g.N[d]) l1 = 0;          // the only tile along d is its own neighbour
+            }
+            l[d][0] = l0;
+            l[d][1] = l1;
+            ok[d][0] = FAST || l0 < ext[d];
+            ok[d][1] = FAST || l1 < ext[d];
+            const float td = (float)(X[d] & fmask) * fr;
+            w[d][0] = 1.f - td;
+            w[d][1] = td;
+        }
+    }
+    // f(offset within the tile, weight, owned)
+    template <class F>
+    __device__ __forceinline__ void each(F f) const
+    {
+#pragma unroll
+        for (int bx = 0; bx < 2; bx++)
+#pragma unroll
+            for (int by = 0; by < 2; by++) {
+                const float wxy = w[0][bx] * w[1][by];
+                const int axy = (l[0][bx] * TY + l[1][by]) * TZ;
+                const bool okxy = ok[0][bx] && ok[1][by];
+#pragma unroll
+                for (int bz = 0; bz < 2; bz++) f(axy + l[2][bz], wxy * w[2][bz], okxy && ok[2][bz]);
+            }
+    }
+};
+
+// shared-memory integer reduction, predicated (no branch around the atomic) or not
+__device__ __forceinline__ void red_shared(int *addr, int v, bool ok, bool always)
+{
+    if (always)
+        asm volatile("red.shared.add.s32 [%0], %1;" ::"r"(smem_u32(addr)), "r"(v) : "memory");
+    else
+        asm volatile("{\n .reg .pred p;\n setp.ne.s32 p, %2, 0;\n @p red.shared.add.s32 [%0], %1;\n}"
+                     ::"r"(smem_u32(addr)), "r"(v), "r"((int)ok)
+                     : "memory");
+}
+
+__device__ __forceinline__ float consumer_max(float v, float *sh /*NCW*/)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
+    if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = v;
+    consumer_sync();
+    float r = sh[0];
+#pragma unroll
+    for (int k = 1; k < NCW; k++) r = fmaxf(r, sh[k]);
+    consumer_sync();
     return r;
 }
+
+// power-of-two exponent e with v <= 2^e (v > 0, normal)
+__device__ __forceinline__ int exp_above(float v) { return (int)((__float_as_uint(v) >> 23) & 255u) - 126; }
 
 // --------------------------------------------------------------------------------------------------
 // scatter
@@ -193,320 +331,404 @@ __constant__ signed char kRuns[14][3] = {{0, 0, 8}, {4, 4, 8}, {2, 2, 4}, {2, 6,
                                          {1, 7, 8}, {6, 6, 8}, {5, 5, 6}, {5, 7, 8}, {3, 3, 4}, {3, 7, 8}, {7, 7, 8}};
 constexpr int NRUNS = 14;
 
-// predicated shared-memory integer reduction: no branch, no divergence region around the atomic
-__device__ __forceinline__ void red_shared_if(int *addr, int v, bool ok)
-{
-    asm volatile("{\n .reg .pred p;\n setp.ne.s32 p, %2, 0;\n @p red.shared.add.s32 [%0], %1;\n}"
-                 ::"r"(smem_u32(addr)), "r"(v), "r"((int)ok)
-                 : "memory");
-}
+struct ScatterSlot {
+    int tile;                   // -1: no more tiles
+    int total;                  // records in all runs
+    int n0;                     // leading records of the tile's own class 0 (all corners inside)
+    int run_start[NRUNS];       // rec index = run_start[r] + flat index
+    int run_prefix[NRUNS + 1];
+};
 
-// deposit one particle into the CTA's tile: each of the 8 corners lands only if this tile owns that mesh point
-template <int C, bool SIGNED>
-__device__ __forceinline__ void deposit(const CicGeom &g, const int t0[3], const int ext[3], uint4 q, const float v[C],
-                                        int (*tile_acc)[TILE_PTS], float fr, unsigned fmask)
-{
-    const unsigned X[3] = {q.x, q.y, q.z};
-    int l[3][2];
-    bool ok[3][2];
-    float w[3][2];
-#pragma unroll
-    for (int d = 0; d < 3; d++) {
-        int l0 = (int)(X[d] >> g.fbits) - t0[d];
-        if (l0 < 0) l0 += g.N[d];          // particle of the low neighbour across the periodic edge
-        int l1 = l0 + 1;
-        if (l1 == g.N[d]) l1 = 0;          // the only tile along d is its own neighbour
-        l[d][0] = l0;
-        l[d][1] = l1;
-        ok[d][0] = l0 < ext[d];
-        ok[d][1] = l1 < ext[d];
-        float td = (float)(X[d] & fmask) * fr;
-        w[d][0] = 1.f - td;
-        w[d][1] = td;
-    }
-#pragma unroll
-    for (int bx = 0; bx < 2; bx++)
-#pragma unroll
-        for (int by = 0; by < 2; by++) {
-            const float wxy = w[0][bx] * w[1][by];
-            const int axy = (l[0][bx] * TY + l[1][by]) * TZ;
-            const bool okxy = ok[0][bx] && ok[1][by];
-#pragma unroll
-            for (int bz = 0; bz < 2; bz++) {
-                const float ww = wxy * w[2][bz];
-                const bool o = okxy && ok[2][bz];
-#pragma unroll
-                for (int c = 0; c < C; c++)
-                    red_shared_if(&tile_acc[c][axy + l[2][bz]], SIGNED ? __float2int_rn(ww * v[c]) : (int)__float2uint_rn(ww * v[c]), o);
-            }
-        }
-}
+template <int C>
+constexpr size_t scatter_smem_bytes() { return (size_t)2 * C * TILE_PTS * sizeof(int) + (size_t)NST * RCAP * sizeof(uint4); }
 
 template <int C, bool HAS_VAL>
-__global__ void __launch_bounds__(256) scatter_kernel(const __grid_constant__ CUtensorMap tmap, CicGeom g,
-                                                      const uint4 *__restrict__ rec, const int *__restrict__ offsets,
-                                                      const float *__restrict__ val, float *__restrict__ mesh)
+__global__ void __launch_bounds__(NTHREADS) scatter_kernel(const __grid_constant__ CUtensorMap tmap, CicGeom g,
+                                                           const uint4 *__restrict__ rec, const int *__restrict__ offsets,
+                                                           const float *__restrict__ val, float *__restrict__ mesh)
 {
-    __shared__ __align__(128) int tile_acc[C][TILE_PTS];
-    __shared__ int run_start[NRUNS + 2];
-    __shared__ int run_prefix[NRUNS + 2];
-    __shared__ float red[32];
+    extern __shared__ __align__(128) unsigned char dsm[];
+    typedef int AccBuf[C][TILE_PTS];
+    AccBuf *acc = reinterpret_cast<AccBuf *>(dsm);                                        // [2]
+    typedef uint4 RecBuf[RCAP];
+    RecBuf *recbuf = reinterpret_cast<RecBuf *>(dsm + (size_t)2 * C * TILE_PTS * sizeof(int));  // [NST]
+    __shared__ __align__(8) unsigned long long full[NST], empty[NST];
+    __shared__ ScatterSlot slot[NST];
+    __shared__ float redf[NCW];
 
-    int t[3], t0[3], ext[3];
-    tile_coords(g, t, t0, ext);
-
-    {
-        int4 *z4 = reinterpret_cast<int4 *>(&tile_acc[0][0]);
-        for (int i = threadIdx.x; i < C * TILE_PTS / 4; i += blockDim.x) z4[i] = make_int4(0, 0, 0, 0);
-    }
-    if (threadIdx.x < 32) {
-        const int r = threadIdx.x;
-        int b = 0, len = 0;
-        if (r < NRUNS) {
-            const int m = kRuns[r][0], c0 = kRuns[r][1], c1 = kRuns[r][2];
-            bool valid = true;
-            int n[3];
-#pragma unroll
-            for (int d = 0; d < 3; d++) {
-                const int low = (m >> (2 - d)) & 1;
-                if (low && g.nt[d] == 1) valid = false;  // the only tile along d is its own neighbour
-                n[d] = t[d] - low;
-                if (n[d] < 0) n[d] += g.nt[d];
-            }
-            if (valid) {
-                const int key = ((n[0] * g.nt[1] + n[1]) * g.nt[2] + n[2]) * NCLS;
-                b = offsets[key + c0];
-                len = offsets[key + c1] - b;
-            }
-        }
-        int inc = len;
-#pragma unroll
-        for (int o = 1; o < 16; o <<= 1) {
-            int u = __shfl_up_sync(0xffffffffu, inc, o);
-            if (r >= o) inc += u;
-        }
-        if (r < NRUNS) {
-            run_start[r] = b - (inc - len);  // so that rec index = run_start[r] + flat index
-            run_prefix[r + 1] = inc;
-        }
-        if (r == 0) run_prefix[0] = 0;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < NST; s++) { mbar_init(&full[s], 32); mbar_init(&empty[s], NCW); }
+        mbar_fence_init();
     }
     __syncthreads();
-    const int own = run_prefix[1], total = run_prefix[NRUNS];
 
-    // flat index -> record (+ values); the own tile is one contiguous run, the 13 neighbour runs are short
-    auto fetch = [&](int i, uint4 &q, float v[C]) {
-        int r = 0;
-        if (i >= own) {
-            r = 1;
-            while (i >= run_prefix[r + 1]) r++;
-        }
-        q = rec[run_start[r] + i];
-        if (HAS_VAL) {
+    if (warp == NCW) {
+        // ---------------- producer warp ----------------
+        // run lookup of a tile: lanes 0..13 read the offsets of their run (the loads of tile n + 1 are issued before
+        // tile n is published, so their latency hides behind the stage wait)
+        auto lookup = [&](int tile, int &b, int &len, int &n0) {
+            b = 0; len = 0; n0 = 0;
+            if (tile < g.ntiles && lane < NRUNS) {
+                int t[3], t0[3], ext[3];
+                tile_coords(g, tile, t, t0, ext);
+                const int m = kRuns[lane][0], c0 = kRuns[lane][1], c1 = kRuns[lane][2];
+                bool valid = true;
+                int nb[3];
 #pragma unroll
-            for (int c = 0; c < C; c++) v[c] = val[(size_t)q.w * C + c];
-        }
-    };
+                for (int d = 0; d < 3; d++) {
+                    const int low = (m >> (2 - d)) & 1;
+                    if (low && g.nt[d] == 1) valid = false;  // the only tile along d is its own neighbour
+                    nb[d] = t[d] - low;
+                    if (nb[d] < 0) nb[d] += g.nt[d];
+                }
+                if (valid) {
+                    const int key = ((nb[0] * g.nt[1] + nb[1]) * g.nt[2] + nb[2]) * NCLS;
+                    b = offsets[key + c0];
+                    len = offsets[key + c1] - b;
+                    if (lane == 0) n0 = offsets[key + 1] - b;
+                }
+            }
+        };
+        TileDraw draw;
+        if (lane == 0) draw.init(g.sched);
+        int tile = 0;
+        if (lane == 0) tile = draw.next(g.sched);
+        tile = __shfl_sync(0xffffffffu, tile, 0);
+        int b, len, n0;
+        lookup(tile, b, len, n0);
+        for (int n = 0;; n++) {
+            int tile_nx = 0;
+            if (lane == 0) tile_nx = draw.next(g.sched);
+            tile_nx = __shfl_sync(0xffffffffu, tile_nx, 0);
+            int b_nx, len_nx, n0_nx;
+            lookup(tile_nx, b_nx, len_nx, n0_nx);
 
-    // the first two rounds (all of a typical tile) are fetched up front and kept in registers
-    const int i0 = threadIdx.x, i1 = threadIdx.x + blockDim.x;
-    uint4 qa = make_uint4(0, 0, 0, 0), qb = qa;
-    float va[C], vb[C];
+            const int s = n % NST;
+            mbar_wait(&empty[s], ((n / NST) & 1) ^ 1);
+            if (tile >= g.ntiles) {
+                if (lane == 0) {
+                    slot[s].tile = -1;
+                    sched_finish(g.sched);
+                }
+                mbar_arrive(&full[s]);
+                break;
+            }
+            int inc = len;
 #pragma unroll
-    for (int c = 0; c < C; c++) va[c] = vb[c] = 0.f;
-    if (i0 < total) fetch(i0, qa, va);
-    if (i1 < total) fetch(i1, qb, vb);
-
-    // bound on the absolute sum any mesh point can reach -> power-of-two fixed-point scale
-    float bound;
-    if (HAS_VAL) {
-        float ma = 0.f, mb = 0.f;
-#pragma unroll
-        for (int c = 0; c < C; c++) { ma = fmaxf(ma, fabsf(va[c])); mb = fmaxf(mb, fabsf(vb[c])); }
-        float part = ma + mb;
-        for (int i = i1 + blockDim.x; i < total; i += blockDim.x) {
-            uint4 q;
-            float v[C];
-            fetch(i, q, v);
-            float m = 0.f;
-#pragma unroll
-            for (int c = 0; c < C; c++) m = fmaxf(m, fabsf(v[c]));
-            part += m;
+            for (int o = 1; o < 16; o <<= 1) {
+                const int u = __shfl_up_sync(0xffffffffu, inc, o);
+                if (lane >= o) inc += u;
+            }
+            const int start = inc - len;
+            const int total = __shfl_sync(0xffffffffu, inc, NRUNS - 1);
+            if (lane < NRUNS) {
+                slot[s].run_start[lane] = b - start;
+                slot[s].run_prefix[lane + 1] = inc;
+            }
+            const int cnt = lane < NRUNS ? max(min(len, RCAP - start), 0) : 0;
+            if (lane == 0) {
+                slot[s].run_prefix[0] = 0;
+                slot[s].tile = tile;
+                slot[s].total = total;
+                slot[s].n0 = n0;
+                // the tile's own run: one bulk copy; the (short) neighbour runs: 16-byte async copies, one lane per run
+                if (cnt > 0) {
+                    mbar_expect_tx(&full[s], (unsigned)cnt * (unsigned)sizeof(uint4));
+                    bulk_load(&recbuf[s][0], rec + b, (unsigned)cnt * (unsigned)sizeof(uint4), &full[s]);
+                } else {
+                    mbar_arrive(&full[s]);
+                }
+            } else {
+                for (int k = 0; k < cnt; k++) cp_async16(&recbuf[s][start + k], rec + b + k);
+                cp_async_arrive(&full[s]);
+            }
+            tile = tile_nx; b = b_nx; len = len_nx; n0 = n0_nx;
         }
-        bound = block_sum(part, red) * 1.0001f;  // margin for the fp32 summation itself
-    } else {
-        bound = (float)total;
+        return;
     }
-    // fixed-point scale: the accumulators cannot overflow because |sum at any point| <= bound, and each of the
-    // <= total deposits at a point rounds by <= 0.5.
-    //   unit mass: deposits are >= 0 -> UNSIGNED accumulation with scale = (2^32 - headroom) / total.  total is an
-    //              integer, so the scale (not a power of two: one extra fp32 rounding per deposit, 6e-8 relative,
-    //              far below the quantum) is the same in every run: the density mesh stays bit-reproducible.
-    //   values:    signed accumulation; bound is an fp32 sum whose last bits depend on the (arbitrary) order of
-    //              the records, so only its exponent is used: scale = 2^(30 - ex) with bound <= 2^ex.
-    float scale;
-    if (HAS_VAL) {
-        const int ex = (int)((__float_as_uint(fmaxf(bound, 1e-37f)) >> 23) & 255u) - 126;
-        const int k = min(30 - ex, 96) - g.kshift;
-        scale = __uint_as_float((unsigned)(127 + k) << 23);
-    } else {
-        const float room = fmaxf(4294967296.f * 0.99999f - (float)total, 1.f);
-        scale = ldexpf(room / fmaxf(bound, 1.f), -g.kshift);
+
+    // ---------------- consumer warps ----------------
+    const int tid = threadIdx.x;
+    {
+        int4 *z4 = reinterpret_cast<int4 *>(&acc[0][0][0]);
+        for (int i = tid; i < 2 * C * TILE_PTS / 4; i += NCT) z4[i] = make_int4(0, 0, 0, 0);
     }
-    const float inv_scale = 1.f / scale;
-    // mean subtraction (unit mass): mq quanta are removed exactly in integer, the sub-quantum rest in fp32
-    long long mq = 0;
-    float mrest = 0.f;
-    if (!HAS_VAL && g.mean != 0.0) {
-        const double m = g.mean * (double)scale;
-        mq = __double2ll_rn(m);
-        mrest = (float)((m - (double)mq) * (double)inv_scale);
-    }
+    consumer_sync();
     const float fr = 1.f / (float)(1u << g.fbits);
     const unsigned fmask = (1u << g.fbits) - 1u;
 
-    auto put = [&](uint4 q, const float vin[C]) {
-        float v[C];
-#pragma unroll
-        for (int c = 0; c < C; c++) v[c] = HAS_VAL ? vin[c] * scale : scale;
-        deposit<C, HAS_VAL>(g, t0, ext, q, v, tile_acc, fr, fmask);
-    };
-    if (i0 < total) put(qa, va);
-    if (i1 < total) put(qb, vb);
-    for (int i = i1 + blockDim.x; i < total; i += blockDim.x) {
-        uint4 q;
-        float v[C];
-        fetch(i, q, v);
-        put(q, v);
-    }
-    __syncthreads();
+    for (int n = 0;; n++) {
+        const int s = n % NST, b = n & 1;
+        mbar_wait(&full[s], (n / NST) & 1);
+        const ScatterSlot &sl = slot[s];
+        const int tile = sl.tile;
+        if (tile < 0) break;
+        const int total = sl.total, n0 = sl.n0;
+        int t[3], t0[3], ext[3];
+        tile_coords(g, tile, t, t0, ext);
 
-    if (g.use_tma) {
-        // int -> float in place (same bytes), then one tensor store per component; TMA clips at the mesh edge
-        int4 *a4 = reinterpret_cast<int4 *>(&tile_acc[0][0]);
-        for (int i = threadIdx.x; i < C * TILE_PTS / 4; i += blockDim.x) {
-            int4 a = a4[i];
-            float4 f = HAS_VAL ? make_float4((float)a.x * inv_scale, (float)a.y * inv_scale, (float)a.z * inv_scale, (float)a.w * inv_scale)
-                               : make_float4((float)((long long)(unsigned)a.x - mq) * inv_scale - mrest, (float)((long long)(unsigned)a.y - mq) * inv_scale - mrest,
-                                             (float)((long long)(unsigned)a.z - mq) * inv_scale - mrest, (float)((long long)(unsigned)a.w - mq) * inv_scale - mrest);
-            reinterpret_cast<float4 *>(a4)[i] = f;
-        }
-        fence_proxy_async_smem();
-        __syncthreads();
-        if (threadIdx.x == 0) {
+        // flat index -> record: the first RCAP are staged in shared memory, the rest come from global
+        auto fetch = [&](int i) -> uint4 {
+            if (i < RCAP) return recbuf[s][i];
+            int r = 0;
+            while (i >= sl.run_prefix[r + 1]) r++;
+            return rec[sl.run_start[r] + i];
+        };
+        auto values = [&](uint4 q, float v[C]) {
 #pragma unroll
-            for (int c = 0; c < C; c++) tma_store_4d(&tmap, &tile_acc[c][0], t0[2], t0[1], t0[0], g.c0 + c);
-            tma_store_commit_and_wait();
-        }
-    } else {
-        // plain path: one warp per z-row
-        const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = blockDim.x >> 5;
-        for (int row = w; row < TX * TY; row += nw) {
-            const int lx = row / TY, ly = row % TY;
-            if (lx < ext[0] && ly < ext[1] && lane < ext[2]) {
-                const size_t o = ((size_t)(t0[0] + lx) * g.N[1] + (t0[1] + ly)) * g.zs + (t0[2] + lane);
+            for (int c = 0; c < C; c++) v[c] = val[(size_t)q.w * C + c];
+        };
+        int *tile_acc = &acc[b][0][0];
+
+        float scale;
+        if (!HAS_VAL) {
+            // unit mass: deposits are >= 0 -> UNSIGNED accumulation with scale = (2^32 - headroom) / total.  total is an
+            // integer, so the scale is the same in every run: the density mesh stays bit-reproducible.  No point can
+            // overflow: sum of weights at a point <= total, and each of the <= total deposits rounds by <= 0.5.
+            const float room = fmaxf(4294967296.f * 0.99999f - (float)total, 1.f);
+            scale = ldexpf(room / fmaxf((float)total, 1.f), -g.kshift);
+            for (int i = tid; i < total; i += NCT) {
+                const uint4 q = fetch(i);
+                if (i < n0) {
+                    Corners<true> cn(g, t0, ext, q, fr, fmask);
+                    cn.each([&](int a, float w, bool) { red_shared(tile_acc + a, (int)__float2uint_rn(w * scale), true, true); });
+                } else {
+                    Corners<false> cn(g, t0, ext, q, fr, fmask);
+                    cn.each([&](int a, float w, bool ok) { red_shared(tile_acc + a, (int)__float2uint_rn(w * scale), ok, false); });
+                }
+            }
+        } else {
+            // values: signed fixed point with a power-of-two scale from a bound on |sum| at any point of the tile.
+            // The bound comes from a first pass that deposits w * max_c|v_c| (unsigned, coarse scale from
+            // total * max|v|); its maximum over the tile, plus the rounding slack, bounds every component's sum.
+            // Integer atomics and a float max only: the result does not depend on the order of the records.
+            const int ia = tid, ib = tid + NCT;
+            uint4 qa = make_uint4(0, 0, 0, 0), qb = qa;
+            float va[C], vb[C];
 #pragma unroll
-                for (int c = 0; c < C; c++) {
-                    const int a = tile_acc[c][row * TZ + lane];
-                    mesh[(size_t)c * g.ms + o] = HAS_VAL ? (float)a * inv_scale : (float)((long long)(unsigned)a - mq) * inv_scale - mrest;
+            for (int c = 0; c < C; c++) va[c] = vb[c] = 0.f;
+            if (ia < total) { qa = fetch(ia); values(qa, va); }
+            if (ib < total) { qb = fetch(ib); values(qb, vb); }
+            float ma = 0.f, mb = 0.f;
+#pragma unroll
+            for (int c = 0; c < C; c++) { ma = fmaxf(ma, fabsf(va[c])); mb = fmaxf(mb, fabsf(vb[c])); }
+            float vmax = fmaxf(ma, mb);
+            for (int i = ib + NCT; i < total; i += NCT) {
+                float v[C];
+                values(fetch(i), v);
+#pragma unroll
+                for (int c = 0; c < C; c++) vmax = fmaxf(vmax, fabsf(v[c]));
+            }
+            vmax = consumer_max(vmax, redf);
+            scale = 1.f;
+            if (total > 0 && vmax > 0.f && vmax < 3e38f) {
+                const float sA = __uint_as_float((unsigned)(127 + min(31 - exp_above(fmaxf((float)total * vmax, 1e-30f)), 96)) << 23);
+                auto pass_a = [&](int i, uint4 q, float m) {
+                    const float ms = m * sA;
+                    if (i < n0) {
+                        Corners<true> cn(g, t0, ext, q, fr, fmask);
+                        cn.each([&](int a, float w, bool) { red_shared(tile_acc + a, (int)__float2uint_rn(w * ms), true, true); });
+                    } else {
+                        Corners<false> cn(g, t0, ext, q, fr, fmask);
+                        cn.each([&](int a, float w, bool ok) { red_shared(tile_acc + a, (int)__float2uint_rn(w * ms), ok, false); });
+                    }
+                };
+                if (ia < total) pass_a(ia, qa, ma);
+                if (ib < total) pass_a(ib, qb, mb);
+                for (int i = ib + NCT; i < total; i += NCT) {
+                    const uint4 q = fetch(i);
+                    float v[C], m = 0.f;
+                    values(q, v);
+#pragma unroll
+                    for (int c = 0; c < C; c++) m = fmaxf(m, fabsf(v[c]));
+                    pass_a(i, q, m);
+                }
+                consumer_sync();
+                unsigned um = 0u;
+                for (int i = tid; i < TILE_PTS; i += NCT) {
+                    um = max(um, (unsigned)tile_acc[i]);
+                    tile_acc[i] = 0;
+                }
+                const float M = consumer_max((float)um * 1.0000002f, redf);  // (float) may round down: one ulp up
+                const float bound = (M + 0.5f * (float)total + 1.f) / sA * 1.001f;
+                const int k = min(30 - exp_above(fmaxf(bound, 1e-37f)), 96) - g.kshift;
+                scale = __uint_as_float((unsigned)(127 + k) << 23);
+                auto pass_b = [&](int i, uint4 q, const float v[C]) {
+                    float vs[C];
+#pragma unroll
+                    for (int c = 0; c < C; c++) vs[c] = v[c] * scale;
+                    if (i < n0) {
+                        Corners<true> cn(g, t0, ext, q, fr, fmask);
+                        cn.each([&](int a, float w, bool) {
+#pragma unroll
+                            for (int c = 0; c < C; c++) red_shared(tile_acc + c * TILE_PTS + a, __float2int_rn(w * vs[c]), true, true);
+                        });
+                    } else {
+                        Corners<false> cn(g, t0, ext, q, fr, fmask);
+                        cn.each([&](int a, float w, bool ok) {
+#pragma unroll
+                            for (int c = 0; c < C; c++) red_shared(tile_acc + c * TILE_PTS + a, __float2int_rn(w * vs[c]), ok, false);
+                        });
+                    }
+                };
+                if (ia < total) pass_b(ia, qa, va);
+                if (ib < total) pass_b(ib, qb, vb);
+                for (int i = ib + NCT; i < total; i += NCT) {
+                    const uint4 q = fetch(i);
+                    float v[C];
+                    values(q, v);
+                    pass_b(i, q, v);
                 }
             }
         }
+        const float inv_scale = 1.f / scale;
+        // mean subtraction (unit mass): mq quanta are removed exactly in integer, the sub-quantum rest in fp32
+        long long mq = 0;
+        float mrest = 0.f;
+        if (!HAS_VAL && g.mean != 0.0) {
+            const double m = g.mean * (double)scale;
+            mq = __double2ll_rn(m);
+            mrest = (float)((m - (double)mq) * (double)inv_scale);
+        }
+
+        if (tid == 0) tma_store_wait_read();  // the previous tile's store has read the other buffer out
+        consumer_sync();                      // all deposits of this tile are in; the other buffer is free
+        if (lane == 0) mbar_arrive(&empty[s]);
+        {
+            // int -> float in place (same bytes), and the other buffer is zeroed for the next tile
+            int4 *a4 = reinterpret_cast<int4 *>(tile_acc);
+            int4 *o4 = reinterpret_cast<int4 *>(&acc[b ^ 1][0][0]);
+            for (int i = tid; i < C * TILE_PTS / 4; i += NCT) {
+                const int4 a = a4[i];
+                float4 f;
+                if (HAS_VAL) {
+                    f = make_float4((float)a.x * inv_scale, (float)a.y * inv_scale, (float)a.z * inv_scale, (float)a.w * inv_scale);
+                } else if (mq == 0) {
+                    f = make_float4((float)(unsigned)a.x * inv_scale, (float)(unsigned)a.y * inv_scale,
+                                    (float)(unsigned)a.z * inv_scale, (float)(unsigned)a.w * inv_scale);
+                } else {
+                    f = make_float4((float)((long long)(unsigned)a.x - mq) * inv_scale - mrest, (float)((long long)(unsigned)a.y - mq) * inv_scale - mrest,
+                                    (float)((long long)(unsigned)a.z - mq) * inv_scale - mrest, (float)((long long)(unsigned)a.w - mq) * inv_scale - mrest);
+                }
+                reinterpret_cast<float4 *>(a4)[i] = f;
+                o4[i] = make_int4(0, 0, 0, 0);
+            }
+        }
+        fence_proxy_async_smem();
+        consumer_sync();
+        if (g.use_tma) {
+            if (tid == 0) {
+#pragma unroll
+                for (int c = 0; c < C; c++) tma_store_4d(&tmap, tile_acc + c * TILE_PTS, t0[2], t0[1], t0[0], g.c0 + c);
+                tma_store_commit();
+            }
+        } else {
+            // plain path: one warp per z-row
+            const float *facc = reinterpret_cast<const float *>(tile_acc);
+            for (int row = warp; row < TX * TY; row += NCW) {
+                const int lx = row / TY, ly = row % TY;
+                if (lx < ext[0] && ly < ext[1] && lane < ext[2]) {
+                    const size_t o = ((size_t)(t0[0] + lx) * g.N[1] + (t0[1] + ly)) * g.zs + (t0[2] + lane);
+#pragma unroll
+                    for (int c = 0; c < C; c++) mesh[(size_t)c * g.ms + o] = facc[c * TILE_PTS + row * TZ + lane];
+                }
+            }
+            consumer_sync();  // the rows are out before anyone zeroes this buffer at the next tile
+        }
     }
+    if (tid == 0) tma_store_wait_all();
 }
 
 // --------------------------------------------------------------------------------------------------
 // gathers
 // --------------------------------------------------------------------------------------------------
+// Measured on B200 (profiles/): TMA tensor loads of these narrow halo boxes (144-byte rows) sustain only about
+// one row per 12 cycles per SM, and a single producer warp issuing 16-byte async copies is issue-bound; 256
+// threads issuing the 16-byte copies themselves (9 per thread and tile) are not.  So the gather is a classic
+// two-stage cp.async pipeline: every thread first starts the copies of the NEXT tile's halo, then interpolates
+// for the particles of the current one.
 enum GatherMode { G_VALUE = 0, G_GRAD = 1, G_FUSED = 2 };
+constexpr int GT = 256;                                    // threads of a gather CTA
+constexpr int GCH = HZP / 4;                               // 16-byte pieces per halo row (9)
+constexpr int GRG = GT / GCH;                              // halo rows covered per pass of the CTA (28)
 
-// KICK: the interpolated acc (and alpha) of a particle is applied on the spot -- p += rn(acc Ka) [+= rn(acc Kb)],
-// x += rn(p D), and for the adjoint xi -= alpha K, pi -= xi D (eq. 16 L172 / eq. 49 L393, same arithmetic and
-// order as kick_drift_kernel) -- and the particle's new sort key is added to the histogram of the next sort, so
-// a step needs no separate kick/drift and histogram passes and acc/alpha never travel through HBM.
-template <int C, int MODE, bool HAS_COT, bool KICK>
-__global__ void __launch_bounds__(256) gather_kernel(const __grid_constant__ CUtensorMap tmap, CicGeom g,
-                                                     const uint4 *__restrict__ rec, const int *__restrict__ offsets,
-                                                     const float *__restrict__ mesh, const float *cot,
-                                                     float cot_scale, float *__restrict__ out, float *__restrict__ out2,
-                                                     PosGeom pg, KickArgs ka)
+struct GatherSlot {
+    int tile;  // -1: no more tiles
+    int beg, end;
+};
+
+constexpr int GST = 2;                                     // halo stages per CTA: GST - 1 tiles in flight while one is computed
+template <int C>
+constexpr size_t gather_smem_bytes() { return (size_t)GST * C * HALO_STRIDE * sizeof(float); }
+
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+// starts the copies of one tile's halo (C meshes) into `halo`; every thread of the CTA takes part
+template <int C>
+__device__ __forceinline__ void halo_issue(const CicGeom &g, const float *__restrict__ mesh, int tile, float *halo)
 {
-    __shared__ __align__(128) float halo[C * HALO_STRIDE];
-    __shared__ __align__(8) unsigned long long bar;
     int t[3], t0[3], ext[3];
-    tile_coords(g, t, t0, ext);
-    const int key0 = ((t[0] * g.nt[1] + t[1]) * g.nt[2] + t[2]) * NCLS;
-    const int beg = offsets[key0], end = offsets[key0 + NCLS];
-    if (beg == end) return;
-
-    // the halo reaches one point past the tile: interior tiles never wrap and can take the TMA box as is
-    const bool interior = g.use_tma && t0[0] + ext[0] < g.N[0] && t0[1] + ext[1] < g.N[1] && t0[2] + ext[2] < g.N[2];
-    uint4 q = make_uint4(0, 0, 0, 0);
-    if (interior) {
-        if (threadIdx.x == 0) mbar_init(&bar, 1);
-        __syncthreads();
-        if (threadIdx.x == 0) {
-            mbar_expect_tx(&bar, (unsigned)(C * HALO_PTS * sizeof(float)));
+    tile_coords(g, tile, t, t0, ext);
+    const bool rows_ok = g.use_tma && (g.N[2] & 3) == 0;  // 16-byte aligned rows
+    if (rows_ok) {
+        // rows (lx, ly), lx <= ext[0], ly <= ext[1], wrapped periodically; along z either HZP contiguous floats or,
+        // at the upper edge, the floats up to the edge plus 4 from z = 0.  thread -> (row of a group of GRG rows,
+        // 16-byte piece); (lx, ly) are carried along, so the loop has no division.
+        const bool zwrap = t0[2] + HZP > g.N[2];
+        const int cpr_main = (zwrap ? g.N[2] - t0[2] : HZP) / 4;
+        const int cpr = cpr_main + (zwrap ? 1 : 0);
+        const int ny = ext[1] + 1, nrow = (ext[0] + 1) * ny;
+        const int rg = threadIdx.x / GCH, ch = threadIdx.x - rg * GCH;
+        if (rg < GRG && ch < cpr) {
+            const int zoff = ch < cpr_main ? t0[2] + ch * 4 : 0;
+            int lx = rg / ny, ly = rg - lx * ny;
+            const int dlx = GRG / ny, dly = GRG - dlx * ny;
+            for (int r = rg; r < nrow; r += GRG) {
+                int gx = t0[0] + lx, gy = t0[1] + ly;
+                if (gx >= g.N[0]) gx -= g.N[0];
+                if (gy >= g.N[1]) gy -= g.N[1];
+                const float *src = mesh + ((size_t)gx * g.N[1] + gy) * g.zs + zoff;
+                float *dst = halo + (lx * HY + ly) * HZP + ch * 4;
 #pragma unroll
-            for (int c = 0; c < C; c++) tma_load_4d(&halo[c * HALO_STRIDE], &tmap, &bar, t0[2], t0[1], t0[0], g.c0 + c);
+                for (int c = 0; c < C; c++) cp_async16(dst + c * HALO_STRIDE, src + (size_t)c * g.ms);
+                lx += dlx;
+                ly += dly;
+                if (ly >= ny) { ly -= ny; lx++; }
+            }
         }
-        if (beg + (int)threadIdx.x < end) q = rec[beg + threadIdx.x];  // overlaps the TMA flight
-        mbar_wait(&bar, 0);
     } else {
-        const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = blockDim.x >> 5;
-        for (int row = w; row < C * HX * HY; row += nw) {
-            const int c = row / (HX * HY), r2 = row % (HX * HY);
+        // meshes whose layout 16-byte copies cannot address: plain loads
+        const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+        for (int r = w; r < C * HX * HY; r += GT / 32) {
+            const int c = r / (HX * HY), r2 = r % (HX * HY);
             const int lx = r2 / HY, ly = r2 % HY;
             if (lx <= ext[0] && ly <= ext[1]) {
                 int gx = t0[0] + lx, gy = t0[1] + ly;
                 if (gx >= g.N[0]) gx -= g.N[0];
                 if (gy >= g.N[1]) gy -= g.N[1];
                 const float *src = mesh + (size_t)c * g.ms + ((size_t)gx * g.N[1] + gy) * g.zs;
-                float *dst = &halo[c * HALO_STRIDE + (lx * HY + ly) * HZP];
-                if (lane <= ext[2]) {
-                    int gz = t0[2] + lane;
+                float *dst = halo + c * HALO_STRIDE + (lx * HY + ly) * HZP;
+                for (int lz = lane; lz <= ext[2]; lz += 32) {
+                    int gz = t0[2] + lz;
                     if (gz >= g.N[2]) gz -= g.N[2];
-                    dst[lane] = src[gz];
-                }
-                if (lane == 0 && ext[2] == TZ) {
-                    int gz = t0[2] + TZ;
-                    if (gz >= g.N[2]) gz -= g.N[2];
-                    dst[TZ] = src[gz];
+                    dst[lz] = src[gz];
                 }
             }
         }
-        if (beg + (int)threadIdx.x < end) q = rec[beg + threadIdx.x];
-        __syncthreads();
     }
+}
 
-    const float fr = 1.f / (float)(1u << g.fbits);
-    const unsigned fmask = (1u << g.fbits) - 1u;
-    for (int i = beg + threadIdx.x; i < end; i += blockDim.x) {
-        if (i != beg + (int)threadIdx.x) q = rec[i];
-        // KICK: the particle's state is fetched first (independent loads, in flight while the weights are formed)
-        long long st_p[3], st_x[3];
-        float st_xi[3];
-        if (KICK) {
-#pragma unroll
-            for (int d = 0; d < 3; d++) {
-                st_p[d] = ka.p[3 * (size_t)q.w + d];
-                if (ka.Ds != 0.0) st_x[d] = ka.x[3 * (size_t)q.w + d];
-                if (MODE == G_FUSED) st_xi[d] = ka.xi[3 * (size_t)q.w + d];
-            }
-        }
-        const unsigned X[3] = {q.x, q.y, q.z};
-        int l[3];
-        float w[3][2];
-#pragma unroll
-        for (int d = 0; d < 3; d++) {
-            l[d] = (int)(X[d] >> g.fbits) - t0[d];
-            float td = (float)(X[d] & fmask) * fr;
-            w[d][0] = 1.f - td;
-            w[d][1] = td;
-        }
-        const int base = (l[0] * HY + l[1]) * HZP + l[2];
-        const size_t j = q.w;
-        float cv[C];
+// per-particle inputs that are fetched one tile ahead
+template <int C, int MODE, bool HAS_COT, bool KICK>
+struct ParticleIn {
+    float cv[C];
+    long long p[3], x[3];
+    float xi[3];
+    __device__ __forceinline__ void load(size_t j, const float *cot, const KickArgs &ka)
+    {
         if (MODE == G_GRAD) {
 #pragma unroll
             for (int c = 0; c < C; c++) cv[c] = HAS_COT ? cot[j * C + c] : 1.f;
@@ -516,88 +738,228 @@ __global__ void __launch_bounds__(256) gather_kernel(const __grid_constant__ CUt
 #pragma unroll
             for (int c = 1; c < C; c++) cv[c] = cot[j * 3 + (c - 1)];
         }
-        float val[C];
-        float gr[3] = {0.f, 0.f, 0.f};
-#pragma unroll
-        for (int c = 0; c < C; c++) val[c] = 0.f;
-#pragma unroll
-        for (int bx = 0; bx < 2; bx++)
-#pragma unroll
-            for (int by = 0; by < 2; by++)
-#pragma unroll
-                for (int bz = 0; bz < 2; bz++) {
-                    const int idx = base + (bx * HY + by) * HZP + bz;
-                    const float W = w[0][bx] * w[1][by] * w[2][bz];
-                    const float dWx = (bx ? 1.f : -1.f) * w[1][by] * w[2][bz];
-                    const float dWy = (by ? 1.f : -1.f) * w[0][bx] * w[2][bz];
-                    const float dWz = (bz ? 1.f : -1.f) * w[0][bx] * w[1][by];
-                    float m = 0.f;  // cotangent-weighted mesh value at this corner
-#pragma unroll
-                    for (int c = 0; c < C; c++) {
-                        const float f = halo[c * HALO_STRIDE + idx];
-                        if (MODE != G_GRAD) val[c] += W * f;
-                        if (MODE != G_VALUE) m += cv[c] * f;
-                    }
-                    if (MODE != G_VALUE) {
-                        gr[0] += dWx * m;
-                        gr[1] += dWy * m;
-                        gr[2] += dWz * m;
-                    }
-                }
         if (KICK) {
-            const float *a3 = MODE == G_FUSED ? &val[1] : &val[0];
-            unsigned int Xn[3];
 #pragma unroll
             for (int d = 0; d < 3; d++) {
-                const size_t i = 3 * j + d;
-                long long pv = st_p[d];
-                if (ka.Ka != 0.0) pv += __double2ll_rn((double)a3[d] * ka.Ka);
-                if (ka.Kb != 0.0) pv += __double2ll_rn((double)a3[d] * ka.Kb);
-                ka.p[i] = pv;
-                if (MODE == G_FUSED) {
-                    float v = st_xi[d];
-                    if (ka.Ka != 0.0) v = fmaf(-gr[d], ka.Kaf, v);
-                    if (ka.Kb != 0.0) v = fmaf(-gr[d], ka.Kbf, v);
-                    ka.xi[i] = v;
-                    if (ka.Ds != 0.0) ka.pi[i] = fmaf(-v, ka.Df, cv[1 + d]);
-                }
-                if (ka.Ds != 0.0) {
-                    const long long xv = st_x[d] + __double2ll_rn((double)pv * ka.Ds);
-                    ka.x[i] = xv;
-                    Xn[d] = record_coord(pg, xv, d);
-                }
-            }
-            if (ka.Ds != 0.0) hist_add(ka.hist, key_of(pg, Xn));
-            if (ka.store) {
-#pragma unroll
-                for (int e = 0; e < 3; e++) {
-                    out[j * 3 + e] = a3[e];
-                    if (MODE == G_FUSED) out2[j * 3 + e] = gr[e];
-                }
-            }
-        } else if (MODE == G_VALUE) {
-#pragma unroll
-            for (int c = 0; c < C; c++) out[j * C + c] = val[c];
-        } else if (MODE == G_GRAD) {
-#pragma unroll
-            for (int e = 0; e < 3; e++) out[j * 3 + e] = gr[e] * cot_scale;
-        } else {
-#pragma unroll
-            for (int e = 0; e < 3; e++) {
-                out[j * 3 + e] = val[1 + e];
-                out2[j * 3 + e] = gr[e];
+                p[d] = ka.p[3 * j + d];
+                if (ka.Ds != 0.0) x[d] = ka.x[3 * j + d];
+                if (MODE == G_FUSED) xi[d] = ka.xi[3 * j + d];
             }
         }
     }
+};
+
+// KICK: the interpolated acc (and alpha) of a particle is applied on the spot -- p += rn(acc Ka) [+= rn(acc Kb)],
+// x += rn(p D), and for the adjoint xi -= alpha K, pi -= xi D (eq. 16 L172 / eq. 49 L393, same arithmetic and
+// order as kick_drift_kernel) -- and the particle's new sort key is added to the histogram of the next sort, so
+// a step needs no separate kick/drift and histogram passes and acc/alpha never travel through HBM.
+template <int C, int MODE, bool HAS_COT, bool KICK>
+__global__ void __launch_bounds__(GT) gather_kernel(CicGeom g, const uint4 *__restrict__ rec, const int *__restrict__ offsets,
+                                                    const float *__restrict__ mesh, const float *cot, float cot_scale,
+                                                    float *__restrict__ out, float *__restrict__ out2, PosGeom pg, KickArgs ka)
+{
+    extern __shared__ __align__(128) unsigned char dsm[];
+    __shared__ GatherSlot slot[8];  // ring of drawn tiles: iteration n computes slot[n & 7] and starts the copies of slot[(n + GST - 1) & 7]
+    auto halo_of = [&](int s) { return reinterpret_cast<float *>(dsm) + (size_t)s * C * HALO_STRIDE; };
+    const int tid = threadIdx.x;
+    typedef ParticleIn<C, MODE, HAS_COT, KICK> PIn;
+
+    // thread 0 draws tiles from the global counter and publishes them two iterations ahead.  The chain
+    // atomic -> offsets -> slot is software-pipelined: every iteration consumes what the previous one requested
+    // (the tile index of the atomic, the offsets of the tile drawn before), so no round trip is exposed.
+    int d_tile = 0, d_beg = 0, d_end = 0, d_atom = 0;  // thread 0 only: tile with offsets in flight; atomic in flight
+    auto draw_request = [&]() {
+        d_tile = d_atom;
+        if (d_tile < g.ntiles) {
+            d_beg = offsets[d_tile * NCLS];
+            d_end = offsets[d_tile * NCLS + NCLS];
+        }
+        d_atom = atomicAdd(&g.sched[0], 1);
+    };
+    auto draw_publish = [&](GatherSlot &dst) {
+        dst.tile = d_tile < g.ntiles ? d_tile : -1;
+        dst.beg = d_beg;
+        dst.end = d_end;
+    };
+    if (tid == 0) {
+        d_atom = atomicAdd(&g.sched[0], 1);
+        draw_request();
+        for (int k = 0; k < GST; k++) {
+            draw_publish(slot[k]);
+            draw_request();
+        }
+    }
+    __syncthreads();
+    for (int k = 0; k < GST - 1; k++) {
+        if (slot[k].tile >= 0 && slot[k].beg < slot[k].end) halo_issue<C>(g, mesh, slot[k].tile, halo_of(k));
+        cp_async_commit();
+    }
+    // first round of the first tile: record and per-particle inputs
+    uint4 q = make_uint4(0, 0, 0, 0);
+    PIn pin;
+    if (slot[0].tile >= 0 && slot[0].beg + tid < slot[0].end) {
+        q = rec[slot[0].beg + tid];
+        pin.load(q.w, cot, ka);
+    }
+
+    const float fr = 1.f / (float)(1u << g.fbits);
+    const unsigned fmask = (1u << g.fbits) - 1u;
+    for (int n = 0;; n++) {
+        const GatherSlot cur = slot[n & 7];
+        if (cur.tile < 0) break;
+        const GatherSlot nxt = slot[(n + 1) & 7];
+        // the halo of the tile GST - 1 iterations ahead starts to fly now (its stage was released by the barrier that
+        // ended iteration n - 1)
+        {
+            const GatherSlot far = slot[(n + GST - 1) & 7];
+            if (far.tile >= 0 && far.beg < far.end && !(g.dbg & 2)) halo_issue<C>(g, mesh, far.tile, halo_of((n + GST - 1) % GST));
+        }
+        cp_async_commit();
+        uint4 q_nx = make_uint4(0, 0, 0, 0);
+        const bool has_nx = nxt.tile >= 0 && nxt.beg + tid < nxt.end;
+        if (has_nx) q_nx = rec[nxt.beg + tid];
+        cp_async_wait<GST - 1>();  // this thread's copies of the current tile have landed ...
+        __syncthreads();     // ... and everybody else's
+
+        int t[3], t0[3], ext[3];
+        tile_coords(g, cur.tile, t, t0, ext);
+        const float *halo = halo_of(n % GST);
+        const int cnt = (g.dbg & 1) ? 0 : cur.end - cur.beg;
+        for (int i = tid; i < cnt; i += GT) {
+            if (i != tid) {
+                q = rec[cur.beg + i];
+                pin.load(q.w, cot, ka);
+            }
+            const size_t j = q.w;
+            const unsigned X[3] = {q.x, q.y, q.z};
+            int l[3];
+            float w[3][2];
+#pragma unroll
+            for (int d = 0; d < 3; d++) {
+                l[d] = (int)(X[d] >> g.fbits) - t0[d];
+                const float td = (float)(X[d] & fmask) * fr;
+                w[d][0] = 1.f - td;
+                w[d][1] = td;
+            }
+            const int base = (l[0] * HY + l[1]) * HZP + l[2];
+            float val[C];
+            float gr[3] = {0.f, 0.f, 0.f};
+#pragma unroll
+            for (int c = 0; c < C; c++) val[c] = 0.f;
+#pragma unroll
+            for (int bx = 0; bx < 2; bx++)
+#pragma unroll
+                for (int by = 0; by < 2; by++)
+#pragma unroll
+                    for (int bz = 0; bz < 2; bz++) {
+                        const int idx = base + (bx * HY + by) * HZP + bz;
+                        const float W = w[0][bx] * w[1][by] * w[2][bz];
+                        const float dWx = (bx ? 1.f : -1.f) * w[1][by] * w[2][bz];
+                        const float dWy = (by ? 1.f : -1.f) * w[0][bx] * w[2][bz];
+                        const float dWz = (bz ? 1.f : -1.f) * w[0][bx] * w[1][by];
+                        float m = 0.f;  // cotangent-weighted mesh value at this corner
+#pragma unroll
+                        for (int c = 0; c < C; c++) {
+                            const float f = halo[c * HALO_STRIDE + idx];
+                            if (MODE != G_GRAD) val[c] += W * f;
+                            if (MODE != G_VALUE) m += pin.cv[c] * f;
+                        }
+                        if (MODE != G_VALUE) {
+                            gr[0] += dWx * m;
+                            gr[1] += dWy * m;
+                            gr[2] += dWz * m;
+                        }
+                    }
+            if (KICK) {
+                const float *a3 = MODE == G_FUSED ? &val[C - 3] : &val[0];
+                unsigned int Xn[3];
+#pragma unroll
+                for (int d = 0; d < 3; d++) {
+                    const size_t i3 = 3 * j + d;
+                    long long pv = pin.p[d];
+                    if (ka.Ka != 0.0) pv += __double2ll_rn((double)a3[d] * ka.Ka);
+                    if (ka.Kb != 0.0) pv += __double2ll_rn((double)a3[d] * ka.Kb);
+                    ka.p[i3] = pv;
+                    if (MODE == G_FUSED) {
+                        float v = pin.xi[d];
+                        if (ka.Ka != 0.0) v = fmaf(-gr[d], ka.Kaf, v);
+                        if (ka.Kb != 0.0) v = fmaf(-gr[d], ka.Kbf, v);
+                        ka.xi[i3] = v;
+                        if (ka.Ds != 0.0) ka.pi[i3] = fmaf(-v, ka.Df, pin.cv[C - 3 + d]);
+                    }
+                    if (ka.Ds != 0.0) {
+                        const long long xv = pin.x[d] + __double2ll_rn((double)pv * ka.Ds);
+                        ka.x[i3] = xv;
+                        Xn[d] = record_coord(pg, xv, d);
+                    }
+                }
+                if (ka.Ds != 0.0) hist_add(ka.hist, key_of(pg, Xn));
+                if (ka.store) {
+#pragma unroll
+                    for (int e = 0; e < 3; e++) {
+                        out[j * 3 + e] = a3[e];
+                        if (MODE == G_FUSED) out2[j * 3 + e] = gr[e];
+                    }
+                }
+            } else if (MODE == G_VALUE) {
+                if ((g.dbg & 4) && val[0] != 12345.f) continue;
+#pragma unroll
+                for (int c = 0; c < C; c++) out[j * C + c] = val[c];
+            } else if (MODE == G_GRAD) {
+#pragma unroll
+                for (int e = 0; e < 3; e++) out[j * 3 + e] = gr[e] * cot_scale;
+            } else {
+#pragma unroll
+                for (int e = 0; e < 3; e++) {
+                    out[j * 3 + e] = val[C - 3 + e];
+                    out2[j * 3 + e] = gr[e];
+                }
+            }
+        }
+        // the next tile's first record has arrived by now: its per-particle inputs are requested before the barrier
+        q = q_nx;
+        if (has_nx) pin.load(q.w, cot, ka);
+        if (tid == 0) {
+            draw_publish(slot[(n + GST) & 7]);
+            draw_request();
+        }
+        __syncthreads();  // stage n % GST may be overwritten; slot[(n + GST) & 7] is published
+    }
+    cp_async_wait<0>();
+    if (tid == 0) sched_finish(g.sched);
 }
 
-static dim3 tile_grid(const Geometry &g) { return dim3((unsigned)g.nt[2], (unsigned)g.nt[1], (unsigned)g.nt[0]); }
-static int env_threads(const char *name, int dflt)
+// --------------------------------------------------------------------------------------------------
+// host: launches
+// --------------------------------------------------------------------------------------------------
+// persistent grid: as many CTAs per SM as the stage buffers and 1536 threads allow, never more CTAs than tiles
+static int persistent_grid(pm_ctx *c, size_t smem_bytes, int threads)
 {
-    const char *e = getenv(name);
-    int v = e ? atoi(e) : dflt;
-    return (v >= 32 && v <= 256 && v % 32 == 0) ? v : dflt;
+    int per_sm = (int)((size_t)(227 * 1024) / (smem_bytes + 2048));
+    const int cap = 1536 / threads;  // 6 gather CTAs (256 threads) or 5 scatter CTAs (288) at most
+    if (per_sm > cap) per_sm = cap;
+    if (per_sm < 1) per_sm = 1;
+    long long n = (long long)c->num_sms * per_sm;
+    if (n > c->g.ntiles) n = c->g.ntiles;
+    return (int)n;
 }
+
+template <class K>
+static cudaError_t allow_smem(K kernel, size_t bytes)
+{
+    return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+}
+
+#define PM_CIC_LAUNCH(ctx, name, kernel, threads, smem, ...)                                          \
+    do {                                                                                     \
+        static bool attr_done_ = false;                                                      \
+        if (!attr_done_) {                                                                   \
+            PM_CUDA(ctx, allow_smem(kernel, smem));                                          \
+            attr_done_ = true;                                                               \
+        }                                                                                    \
+        kernel<<<persistent_grid(ctx, smem, threads), threads, smem, (ctx)->stream>>>(__VA_ARGS__); \
+        PM_LAUNCH_CHECK(ctx, name);                                                          \
+    } while (0)
 
 int scatter_sorted(pm_ctx *c, const float *val, int C, float *mesh, int zs, long long ms, double mean)
 {
@@ -605,21 +967,17 @@ int scatter_sorted(pm_ctx *c, const float *val, int C, float *mesh, int zs, long
     CicGeom g = make_cic_geom(c, mesh, C, zs, ms, true, &map);
     g.mean = (C == 1 && !val) ? mean : 0.0;
     double np = (double)c->cur_np, ng = (double)c->g.ng;
-    dim3 grid = tile_grid(c->g);
     if (C == 1 && !val) {
         Timer t(c, TC_SCATTER1, 12.0 * np + 4.0 * ng);
-        scatter_kernel<1, false><<<grid, env_threads("PM_SCATTER_THREADS", 128), 0, c->stream>>>(map, g, c->rec, c->offsets, nullptr, mesh);
-        PM_LAUNCH_CHECK(c, "scatter_kernel<1>");
+        PM_CIC_LAUNCH(c, "scatter_kernel<1>", (scatter_kernel<1, false>), NTHREADS, scatter_smem_bytes<1>(), map, g, c->rec, c->offsets, nullptr, mesh);
         t.stop();
     } else if (C == 1) {
         Timer t(c, TC_SCATTER1, 16.0 * np + 4.0 * ng);
-        scatter_kernel<1, true><<<grid, env_threads("PM_SCATTER_THREADS", 128), 0, c->stream>>>(map, g, c->rec, c->offsets, val, mesh);
-        PM_LAUNCH_CHECK(c, "scatter_kernel<1,val>");
+        PM_CIC_LAUNCH(c, "scatter_kernel<1,val>", (scatter_kernel<1, true>), NTHREADS, scatter_smem_bytes<1>(), map, g, c->rec, c->offsets, val, mesh);
         t.stop();
     } else if (C == 3 && val) {
         Timer t(c, TC_SCATTER3, 24.0 * np + 12.0 * ng);
-        scatter_kernel<3, true><<<grid, env_threads("PM_SCATTER_THREADS", 256), 0, c->stream>>>(map, g, c->rec, c->offsets, val, mesh);
-        PM_LAUNCH_CHECK(c, "scatter_kernel<3,val>");
+        PM_CIC_LAUNCH(c, "scatter_kernel<3,val>", (scatter_kernel<3, true>), NTHREADS, scatter_smem_bytes<3>(), map, g, c->rec, c->offsets, val, mesh);
         t.stop();
     } else {
         return fail(c, PM_EINVAL, "scatter", "C must be 1, or 3 with values");
@@ -640,25 +998,21 @@ int gather_sorted(pm_ctx *c, const float *mesh, int C, int zs, long long ms, flo
     CUtensorMap map;
     CicGeom g = make_cic_geom(c, mesh, C, zs, ms, false, &map);
     double np = (double)c->cur_np, ng = (double)c->g.ng;
-    dim3 grid = tile_grid(c->g);
     PosGeom pg = make_pos_geom(c->g);
     KickArgs none;
     memset(&none, 0, sizeof none);
     if (ka && C != 3) return fail(c, PM_EINVAL, "gather", "internal: kick needs C = 3");
     if (C == 1) {
         Timer t(c, TC_GATHER3, 16.0 * np + 4.0 * ng);
-        gather_kernel<1, G_VALUE, false, false><<<grid, env_threads("PM_GATHER_THREADS", 256), 0, c->stream>>>(map, g, c->rec, c->offsets, mesh, nullptr, 1.f, out, nullptr, pg, none);
-        PM_LAUNCH_CHECK(c, "gather_kernel<1>");
+        PM_CIC_LAUNCH(c, "gather_kernel<1>", (gather_kernel<1, G_VALUE, false, false>), GT, gather_smem_bytes<1>(), g, c->rec, c->offsets, mesh, nullptr, 1.f, out, nullptr, pg, none);
         t.stop();
     } else if (C == 3 && !ka) {
         Timer t(c, TC_GATHER3, 24.0 * np + 12.0 * ng);
-        gather_kernel<3, G_VALUE, false, false><<<grid, env_threads("PM_GATHER_THREADS", 256), 0, c->stream>>>(map, g, c->rec, c->offsets, mesh, nullptr, 1.f, out, nullptr, pg, none);
-        PM_LAUNCH_CHECK(c, "gather_kernel<3>");
+        PM_CIC_LAUNCH(c, "gather_kernel<3>", (gather_kernel<3, G_VALUE, false, false>), GT, gather_smem_bytes<3>(), g, c->rec, c->offsets, mesh, nullptr, 1.f, out, nullptr, pg, none);
         t.stop();
     } else if (C == 3) {
         Timer t(c, TC_GATHER_KICK, (12.0 + kick_bytes(ka, false)) * np + 12.0 * ng);
-        gather_kernel<3, G_VALUE, false, true><<<grid, env_threads("PM_GATHER_THREADS", 256), 0, c->stream>>>(map, g, c->rec, c->offsets, mesh, nullptr, 1.f, out, nullptr, pg, *ka);
-        PM_LAUNCH_CHECK(c, "gather_kernel<3,kick>");
+        PM_CIC_LAUNCH(c, "gather_kernel<3,kick>", (gather_kernel<3, G_VALUE, false, true>), GT, gather_smem_bytes<3>(), g, c->rec, c->offsets, mesh, nullptr, 1.f, out, nullptr, pg, *ka);
         t.stop();
     } else {
         return fail(c, PM_EINVAL, "gather", "C must be 1 or 3");
@@ -672,23 +1026,19 @@ int gather_grad_sorted(pm_ctx *c, const float *mesh, int C, int zs, long long ms
     CUtensorMap map;
     CicGeom g = make_cic_geom(c, mesh, C, zs, ms, false, &map);
     double np = (double)c->cur_np, ng = (double)c->g.ng;
-    dim3 grid = tile_grid(c->g);
     PosGeom pg = make_pos_geom(c->g);
     KickArgs none;
     memset(&none, 0, sizeof none);
-    const int th = env_threads("PM_GATHER_THREADS", 256);
+    if (C != 1 && C != 3) return fail(c, PM_EINVAL, "gather_grad", "C must be 1 or 3");
     Timer t(c, TC_GATHER_GRAD, (24.0 + (cot ? 4.0 * C : 0.0)) * np + 4.0 * C * ng);
     if (C == 1 && !cot)
-        gather_kernel<1, G_GRAD, false, false><<<grid, th, 0, c->stream>>>(map, g, c->rec, c->offsets, mesh, nullptr, cot_scale, out, nullptr, pg, none);
+        PM_CIC_LAUNCH(c, "gather_kernel<1,grad>", (gather_kernel<1, G_GRAD, false, false>), GT, gather_smem_bytes<1>(), g, c->rec, c->offsets, mesh, nullptr, cot_scale, out, nullptr, pg, none);
     else if (C == 1)
-        gather_kernel<1, G_GRAD, true, false><<<grid, th, 0, c->stream>>>(map, g, c->rec, c->offsets, mesh, cot, cot_scale, out, nullptr, pg, none);
-    else if (C == 3 && !cot)
-        gather_kernel<3, G_GRAD, false, false><<<grid, th, 0, c->stream>>>(map, g, c->rec, c->offsets, mesh, nullptr, cot_scale, out, nullptr, pg, none);
-    else if (C == 3)
-        gather_kernel<3, G_GRAD, true, false><<<grid, th, 0, c->stream>>>(map, g, c->rec, c->offsets, mesh, cot, cot_scale, out, nullptr, pg, none);
+        PM_CIC_LAUNCH(c, "gather_kernel<1,grad,cot>", (gather_kernel<1, G_GRAD, true, false>), GT, gather_smem_bytes<1>(), g, c->rec, c->offsets, mesh, cot, cot_scale, out, nullptr, pg, none);
+    else if (!cot)
+        PM_CIC_LAUNCH(c, "gather_kernel<3,grad>", (gather_kernel<3, G_GRAD, false, false>), GT, gather_smem_bytes<3>(), g, c->rec, c->offsets, mesh, nullptr, cot_scale, out, nullptr, pg, none);
     else
-        return fail(c, PM_EINVAL, "gather_grad", "C must be 1 or 3");
-    PM_LAUNCH_CHECK(c, "gather_kernel<grad>");
+        PM_CIC_LAUNCH(c, "gather_kernel<3,grad,cot>", (gather_kernel<3, G_GRAD, true, false>), GT, gather_smem_bytes<3>(), g, c->rec, c->offsets, mesh, cot, cot_scale, out, nullptr, pg, none);
     t.stop();
     return PM_OK;
 }
@@ -700,18 +1050,15 @@ int gather_fused_sorted(pm_ctx *c, const float *mesh4, int zs, long long ms, con
     CicGeom g = make_cic_geom(c, mesh4, 4, zs, ms, false, &map);
     double np = (double)c->cur_np, ng = (double)c->g.ng;
     PosGeom pg = make_pos_geom(c->g);
-    const int th = env_threads("PM_GATHER_THREADS", 256);
     if (!ka) {
         KickArgs none;
         memset(&none, 0, sizeof none);
         Timer t(c, TC_GATHER_FUSED, 48.0 * np + 16.0 * ng);
-        gather_kernel<4, G_FUSED, true, false><<<tile_grid(c->g), th, 0, c->stream>>>(map, g, c->rec, c->offsets, mesh4, pi, 1.f, acc, alpha, pg, none);
-        PM_LAUNCH_CHECK(c, "gather_kernel<fused>");
+        PM_CIC_LAUNCH(c, "gather_kernel<fused>", (gather_kernel<4, G_FUSED, true, false>), GT, gather_smem_bytes<4>(), g, c->rec, c->offsets, mesh4, pi, 1.f, acc, alpha, pg, none);
         t.stop();
     } else {
         Timer t(c, TC_GATHER_FUSED, (24.0 + kick_bytes(ka, true)) * np + 16.0 * ng);
-        gather_kernel<4, G_FUSED, true, true><<<tile_grid(c->g), th, 0, c->stream>>>(map, g, c->rec, c->offsets, mesh4, pi, 1.f, acc, alpha, pg, *ka);
-        PM_LAUNCH_CHECK(c, "gather_kernel<fused,kick>");
+        PM_CIC_LAUNCH(c, "gather_kernel<fused,kick>", (gather_kernel<4, G_FUSED, true, true>), GT, gather_smem_bytes<4>(), g, c->rec, c->offsets, mesh4, pi, 1.f, acc, alpha, pg, *ka);
         t.stop();
     }
     return PM_OK;

@@ -84,6 +84,8 @@ struct pm_ctx {
     int *hist;                   // nkeys + 1 key histogram; zero between sorts (the scan clears it)
     unsigned long long *scan_agg;  // scan scratch: per-block totals tagged with the launch epoch
     unsigned int scan_epoch;
+    int *sched;                  // 2 ints: tile counter and finished-CTA count of the persistent CIC kernels (zero between launches)
+    int num_sms;
     long long *x;                // [np][3] int64 absolute position (q + s) * 2^XBITS, not wrapped
     long long *p;                // [np][3] int64 momentum * 2^PBITS
     float *acc, *xi, *pi, *alpha;  // [np][3]
