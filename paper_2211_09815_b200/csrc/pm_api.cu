@@ -11,7 +11,7 @@ namespace pm {
 
 const char *const kTimingNames[TC_NCLASSES] = {
     "bin_count", "bin_scan", "bin_reorder", "scatter1", "scatter3", "gather", "gather_grad", "gather_fused", "gather_kick",
-    "kspace_force", "kspace_adjoint", "fft_r2c", "fft_c2r", "kick_drift", "objective", "convert"};
+    "kspace_force", "kspace_adjoint", "fft_r2c", "fft_c2r", "fft_z_r2c", "fft_z_c2r", "fft_y", "kick_drift", "objective", "convert"};
 
 static thread_local std::string g_err_noctx;
 
@@ -137,12 +137,14 @@ static size_t carve_workspace(pm_ctx *c, const Geometry &g, void *base)
     int tabn = g.N[0] > g.N[1] ? g.N[0] : g.N[1];
     if (g.N[2] > tabn) tabn = g.N[2];
     double *ktab = w.take<double>((size_t)9 * tabn);
+    void *ffttab = w.take<char>(fft_own_table_bytes(g));
     void *fftw = w.take<char>(fft_work_reserve(g));
     if (c) {
         for (int k = 0; k < 7; k++) c->mesh[k] = m + (size_t)k * g.mesh_stride;
         c->rec = rec; c->offsets = offsets; c->cursor = cursor; c->hist = hist; c->sched = sched; c->scan_agg = scan_agg;
         c->x = x; c->p = p; c->acc = acc; c->xi = xi; c->pi = pi; c->alpha = alpha;
         c->scal = scal; c->ktab = ktab; c->ktabn = tabn;
+        c->fft_tab = ffttab;
         c->fft_work = fftw; c->fft_work_bytes = fft_work_reserve(g);
     }
     return w.off;
@@ -212,8 +214,11 @@ static int upload_ktab(pm_ctx *c)
     const double PI = 3.14159265358979323846264338327950288;
     for (int d = 0; d < 3; d++) {
         int N = g.N[d];
+        std::vector<int> order;  // frequency index held at memory position i (digit-reversed for the own FFT's x, y)
+        fft_own_axis_order(c, d, order);
         for (int i = 0; i < N; i++) {
-            int m = i < (N + 1) / 2 ? i : i - N;
+            int fi = order[i];
+            int m = fi < (N + 1) / 2 ? fi : fi - N;
             double k = 2.0 * PI * (double)m / (double)N;
             bool nyq = (N % 2 == 0) && (m == -N / 2);
             double dec = 1.0;
@@ -300,9 +305,11 @@ int pm_init(pm_ctx **out, const pm_params *params, void *dev_workspace, size_t b
     }
     carve_workspace(c, g, dev_workspace);
     c->tma_ok = false;
-    rc = make_plans(c);
+    c->own_fft = fft_own_supported(g);
+    rc = c->own_fft ? PM_OK : make_plans(c);
     if (rc == PM_OK) rc = cic_init_tensor_maps(c);
     if (rc == PM_OK) rc = upload_ktab(c);
+    if (rc == PM_OK) rc = fft_own_init(c);
     c->scan_epoch = 0;
     {
         int dev = 0;

@@ -1,0 +1,632 @@
+// pm_fft.cu -- own 3-D FFT passes with the k-space operators fused into the x pass (power-of-two meshes).
+//
+// PAPER.md L127-131 (eq. 11): the force costs "4 (1 forward and 3 inverse) FFTs"; with a library FFT that is
+// 4 x 3 passes over the mesh plus the Green's-function kernel.  Here the transform along x, the multiplication
+// by  i kt_d G(k)  (eq. 11; pm_kspace.cu states the operators) and the three inverse transforms along x are ONE
+// kernel: a CTA holds a tile of x-columns in shared memory, transforms it, and writes the three force components
+// already transformed back along x.  A force evaluation then moves
+//     z R2C (1r + 1w), y (1r + 1w), x fused (1r + 3w), 3 x y^-1 (3r + 3w), 3 x z^-1 C2R (3r + 3w) = 20 mesh transfers
+// instead of 28 with cuFFT (4 transforms x 3 passes x 2 + the 1r + 3w k-space kernel); the adjoint operator
+// (3 meshes in, 1 out; transpose of eq. 11) is fused the same way.
+//
+// The 1-D transforms are Stockham-free in-place decimation-in-frequency stages of radix 16/8/4/2 on a shared-memory
+// tile [position][column]: a thread loads R elements of one column into registers, runs an R-point DFT there,
+// applies the stage twiddles (fp64-built table) and stores.  Forward stages leave the spectrum in digit-reversed
+// order along x and y; the inverse runs the inverse stages in reverse order, so no reordering pass exists:
+// only the per-axis k tables (kt, k^2, deconvolution) are stored in that permuted order.  z is kept in natural
+// order (the real <-> half-complex pre/post-processing pairs k with N/2 - k inside the tile anyway).
+// Conventions as cuFFT: forward e^{-ikg} unnormalised, inverse unnormalised (1/N_g is folded into G, R13).
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+
+#include "pm_internal.cuh"
+
+namespace pm {
+
+// ---- R-point DFT in registers ----------------------------------------------------------------------------
+__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
+__device__ __forceinline__ float2 cmul(float2 a, float2 b) { return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
+__device__ __forceinline__ float2 cmulc(float2 a, float2 b) { return make_float2(a.x * b.x + a.y * b.y, a.y * b.x - a.x * b.y); }  // a * conj(b)
+
+// d * exp(-+ 2 pi i idx / 16); idx is a compile-time constant after unrolling
+template <bool INV>
+__device__ __forceinline__ float2 mul_w16(float2 d, int idx)
+{
+    const float c1 = 0.92387953251128674f, s1 = 0.38268343236508977f, h = 0.70710678118654752f;
+    float c, s;
+    switch (idx) {
+        case 0: return d;
+        case 1: c = c1; s = s1; break;
+        case 2: c = h; s = h; break;
+        case 3: c = s1; s = c1; break;
+        case 4: return INV ? make_float2(-d.y, d.x) : make_float2(d.y, -d.x);
+        case 5: c = -s1; s = c1; break;
+        case 6: c = -h; s = h; break;
+        default: c = -c1; s = s1; break;
+    }
+    // forward: (c - i s); inverse: (c + i s)
+    return INV ? make_float2(d.x * c - d.y * s, d.y * c + d.x * s) : make_float2(d.x * c + d.y * s, d.y * c - d.x * s);
+}
+
+__host__ __device__ constexpr int bitrev(int i, int R)
+{
+    int r = 0;
+    for (int b = 1; b < R; b <<= 1) { r = (r << 1) | (i & 1); i >>= 1; }
+    return r;
+}
+
+// in place; natural order in, v[i] = X[bitrev(i)] out
+template <int R, bool INV>
+__device__ __forceinline__ void reg_dft(float2 (&v)[R])
+{
+#pragma unroll
+    for (int len = R; len >= 2; len >>= 1) {
+        const int half = len >> 1;
+#pragma unroll
+        for (int b = 0; b < R; b += len) {
+#pragma unroll
+            for (int j = 0; j < half; j++) {
+                const float2 a = v[b + j], c = v[b + j + half];
+                v[b + j] = cadd(a, c);
+                v[b + j + half] = mul_w16<INV>(csub(a, c), j * (16 / len));
+            }
+        }
+    }
+}
+
+constexpr int FFT_T = 256;  // threads per CTA of every FFT kernel
+
+// ---- one transform along the tile's position axis, everything but the data known at compile time -----------
+// tile [N][PITCH] (float2), columns [0, ncol) of 1 << CS; tw = exp(-2 pi i k / N), k < N (shared memory).
+// Stage of span L, radix R = min(16, L): butterfly (blk, j) takes positions blk L + j + m L/R, m < R.
+template <int N, int L, bool INV, int PITCH, int CS>
+__device__ __forceinline__ void fft_stage(float2 *tile, int ncol, const float2 *tw)
+{
+    constexpr int R = L >= 16 ? 16 : L;
+    constexpr int Lr = L / R, twstep = N / L;
+    constexpr int nwork = (N / R) << CS;
+#pragma unroll 1
+    for (int wk = threadIdx.x; wk < nwork; wk += FFT_T) {
+        const int col = wk & ((1 << CS) - 1);
+        if (col >= ncol) continue;
+        const int bf = wk >> CS;
+        const int blk = bf / Lr, j = bf - blk * Lr;
+        float2 *p = tile + (blk * L + j) * PITCH + col;
+        float2 v[R];
+#pragma unroll
+        for (int m = 0; m < R; m++) v[m] = p[m * Lr * PITCH];
+        if (INV && Lr > 1) {
+#pragma unroll
+            for (int q = 1; q < R; q++) v[q] = cmulc(v[q], tw[j * q * twstep]);
+        }
+        reg_dft<R, INV>(v);
+#pragma unroll
+        for (int i = 0; i < R; i++) {
+            const int q = bitrev(i, R);
+            float2 o = v[i];
+            if (!INV && Lr > 1 && q != 0) o = cmul(o, tw[j * q * twstep]);
+            p[q * Lr * PITCH] = o;
+        }
+    }
+}
+
+template <int N, int L, bool INV, int PITCH, int CS>
+struct AxisFFT {
+    static constexpr int R = L >= 16 ? 16 : L;
+    static __device__ __forceinline__ void run(float2 *tile, int ncol, const float2 *tw)
+    {
+        if (!INV) {
+            fft_stage<N, L, false, PITCH, CS>(tile, ncol, tw);
+            __syncthreads();
+            AxisFFT<N, L / R, INV, PITCH, CS>::run(tile, ncol, tw);
+        } else {
+            AxisFFT<N, L / R, INV, PITCH, CS>::run(tile, ncol, tw);
+            fft_stage<N, L, true, PITCH, CS>(tile, ncol, tw);
+            __syncthreads();
+        }
+    }
+};
+template <int N, bool INV, int PITCH, int CS>
+struct AxisFFT<N, 1, INV, PITCH, CS> {
+    static __device__ __forceinline__ void run(float2 *, int, const float2 *) {}
+};
+
+// host mirror of the stage sequence (for the position <-> frequency tables)
+struct AxisPlan {
+    int N;
+    int nst;
+    int radix[4];
+    int span[4];
+};
+
+// ---- device-side description of the mesh in k-space layout --------------------------------------------------
+struct FftGeom {
+    int N[3];
+    int zsc;             // complex elements per z-row in memory (zs / 2); columns [0, zsc) are moved, Nz/2 + 1 are meaningful
+    long long cstride;   // complex elements per mesh
+    const float2 *twx, *twy, *twz;   // exp(-2 pi i k / N) for N = Nx, Ny, Nz/2
+    const float2 *twzr;  // exp(-2 pi i k / Nz), k = 0 .. Nz/2: real <-> half-complex post-processing
+    const int *posz;     // position of frequency k after the forward stages of the Nz/2-point transform
+    const double *ktab;  // [3 axes][3: kt, k^2, dec][tabn] in MEMORY order (x, y digit-reversed, z natural)
+    int tabn;
+    double c0;           // 3/2 Om / (nbar N_g)
+};
+
+constexpr int ZROWS = 16;   // z-rows per CTA of the real <-> half-complex passes
+constexpr int ZP = ZROWS + 1;
+
+__device__ __forceinline__ void fft_cp_async16(void *dst, const void *src)
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(dst)), "l"((unsigned long long)src) : "memory");
+}
+__device__ __forceinline__ void fft_cp_async_wait_all() { asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;" ::: "memory"); }
+
+// global -> tile [N][1 << CS]: element (pos, col) from base[pos * stride + col]; 16-byte async copies (column pairs;
+// ncol is even: 16, 8 or the 2 columns of the last tile)
+template <int N, int CS>
+__device__ __forceinline__ void tile_load(float2 *tile, const float2 *base, long long stride, int ncol)
+{
+    constexpr int HB = 1 << (CS - 1);  // column pairs per position
+    const int cp = threadIdx.x & (HB - 1);
+    if (2 * cp < ncol) {
+#pragma unroll 4
+        for (int pos = threadIdx.x >> (CS - 1); pos < N; pos += FFT_T >> (CS - 1))
+            fft_cp_async16(tile + (pos << CS) + 2 * cp, base + (size_t)pos * stride + 2 * cp);
+    }
+}
+template <int N, int CS>
+__device__ __forceinline__ void tile_store(const float2 *tile, float2 *base, long long stride, int ncol)
+{
+    constexpr int HB = 1 << (CS - 1);
+    const int cp = threadIdx.x & (HB - 1);
+    if (2 * cp < ncol) {
+#pragma unroll 4
+        for (int pos = threadIdx.x >> (CS - 1); pos < N; pos += FFT_T >> (CS - 1))
+            *reinterpret_cast<float4 *>(base + (size_t)pos * stride + 2 * cp) = *reinterpret_cast<const float4 *>(tile + (pos << CS) + 2 * cp);
+    }
+}
+__device__ __forceinline__ void load_tw(float2 *dst, const float2 *src, int n)
+{
+    for (int i = threadIdx.x; i < n; i += FFT_T) dst[i] = src[i];
+}
+
+// ---- y pass: in-place transform along y of nb meshes ---------------------------------------------------------
+// grid = (column tiles along z, Nx, nb); dynamic shared memory: tile [Ny][1 << CS] + Ny twiddles
+template <int NY, int CS, bool INV>
+__global__ void __launch_bounds__(FFT_T) fft_y_kernel(FftGeom g, float2 *data)
+{
+    extern __shared__ __align__(16) unsigned char fsm[];
+    float2 *tile = reinterpret_cast<float2 *>(fsm);
+    float2 *tw = tile + (NY << CS);
+    constexpr int B = 1 << CS;
+    const int col0 = blockIdx.x * B, ncol = min(B, g.zsc - col0);
+    float2 *base = data + (size_t)blockIdx.z * g.cstride + (size_t)blockIdx.y * NY * g.zsc + col0;
+    tile_load<NY, CS>(tile, base, g.zsc, ncol);
+    load_tw(tw, g.twy, NY);
+    fft_cp_async_wait_all();
+    __syncthreads();
+    AxisFFT<NY, NY, INV, B, CS>::run(tile, ncol, tw);
+    tile_store<NY, CS>(tile, base, g.zsc, ncol);
+}
+
+// G(k) of one mode from the per-axis tables in memory order (fp64, rounded to fp32 once); G(0) = 0 (R9)
+__device__ __forceinline__ float mode_green(const FftGeom &g, int ix, int iy, int iz)
+{
+    const double *tx = g.ktab, *ty = g.ktab + 3 * g.tabn, *tz = g.ktab + 6 * g.tabn;
+    const double k2 = tx[g.tabn + ix] + ty[g.tabn + iy] + tz[g.tabn + iz];
+    const double dec = tx[2 * g.tabn + ix] * ty[2 * g.tabn + iy] * tz[2 * g.tabn + iz];
+    return k2 > 0.0 ? (float)(g.c0 * dec / k2) : 0.f;
+}
+
+// ---- x pass fused with the force operator: rho(k) -> f_d(k) = i kt_d G rho(k), d = 1..3, back-transformed along x ----
+// grid = (column tiles along z, Ny); shared: spectrum tile + work tile + Nx twiddles + Nx kt_x
+template <int NX, int CS>
+__global__ void __launch_bounds__(FFT_T) fft_x_force_kernel(FftGeom g, const float2 *rho, float2 *f)
+{
+    extern __shared__ __align__(16) unsigned char fsm[];
+    constexpr int B = 1 << CS;
+    float2 *spec = reinterpret_cast<float2 *>(fsm);
+    float2 *work = spec + (NX << CS);
+    float2 *tw = work + (NX << CS);
+    float *ktx = reinterpret_cast<float *>(tw + NX);
+    const int col0 = blockIdx.x * B, ncol = min(B, g.zsc - col0);
+    const int iy = blockIdx.y;
+    const long long stride = (long long)g.N[1] * g.zsc;
+    const size_t off = (size_t)iy * g.zsc + col0;
+    tile_load<NX, CS>(spec, rho + off, stride, ncol);
+    load_tw(tw, g.twx, NX);
+    for (int i = threadIdx.x; i < NX; i += FFT_T) ktx[i] = (float)g.ktab[i];
+    fft_cp_async_wait_all();
+    __syncthreads();
+    AxisFFT<NX, NX, false, B, CS>::run(spec, ncol, tw);
+    // Green's function once per mode, in place
+    const int col = threadIdx.x & (B - 1);
+    const int iz = min(col0 + col, g.N[2] / 2);
+    const float kty = (float)g.ktab[3 * g.tabn + iy], ktz = (float)g.ktab[6 * g.tabn + iz];
+    if (col < ncol) {
+#pragma unroll 4
+        for (int pos = threadIdx.x >> CS; pos < NX; pos += FFT_T >> CS) {
+            const float G = mode_green(g, pos, iy, iz);
+            float2 r = spec[(pos << CS) + col];
+            spec[(pos << CS) + col] = make_float2(G * r.x, G * r.y);
+        }
+    }
+    // (no barrier needed: every thread re-reads only the elements it has just written)
+#pragma unroll 1
+    for (int d = 0; d < 3; d++) {
+        if (col < ncol) {
+#pragma unroll 4
+            for (int pos = threadIdx.x >> CS; pos < NX; pos += FFT_T >> CS) {
+                const float c = d == 0 ? ktx[pos] : (d == 1 ? kty : ktz);
+                const float2 r = spec[(pos << CS) + col];
+                work[(pos << CS) + col] = make_float2(-c * r.y, c * r.x);  // times +i kt_d
+            }
+        }
+        __syncthreads();
+        AxisFFT<NX, NX, true, B, CS>::run(work, ncol, tw);
+        tile_store<NX, CS>(work, f + (size_t)d * g.cstride + off, stride, ncol);
+        __syncthreads();
+    }
+}
+
+// ---- x pass fused with the adjoint operator: psi(k) = -i G sum_d kt_d Pi_d(k), back-transformed along x ----------
+template <int NX, int CS>
+__global__ void __launch_bounds__(FFT_T) fft_x_adjoint_kernel(FftGeom g, const float2 *Pi, float2 *psi)
+{
+    extern __shared__ __align__(16) unsigned char fsm[];
+    constexpr int B = 1 << CS;
+    float2 *accum = reinterpret_cast<float2 *>(fsm);
+    float2 *work = accum + (NX << CS);
+    float2 *tw = work + (NX << CS);
+    float *ktx = reinterpret_cast<float *>(tw + NX);
+    const int col0 = blockIdx.x * B, ncol = min(B, g.zsc - col0);
+    const int iy = blockIdx.y;
+    const long long stride = (long long)g.N[1] * g.zsc;
+    const size_t off = (size_t)iy * g.zsc + col0;
+    const int col = threadIdx.x & (B - 1);
+    const int iz = min(col0 + col, g.N[2] / 2);
+    const float kty = (float)g.ktab[3 * g.tabn + iy], ktz = (float)g.ktab[6 * g.tabn + iz];
+    load_tw(tw, g.twx, NX);
+    for (int i = threadIdx.x; i < NX; i += FFT_T) ktx[i] = (float)g.ktab[i];
+#pragma unroll 1
+    for (int d = 0; d < 3; d++) {
+        tile_load<NX, CS>(work, Pi + (size_t)d * g.cstride + off, stride, ncol);
+        fft_cp_async_wait_all();
+        __syncthreads();
+        AxisFFT<NX, NX, false, B, CS>::run(work, ncol, tw);
+        if (col < ncol) {
+#pragma unroll 4
+            for (int pos = threadIdx.x >> CS; pos < NX; pos += FFT_T >> CS) {
+                const float c = d == 0 ? ktx[pos] : (d == 1 ? kty : ktz);
+                const float2 v = work[(pos << CS) + col];
+                float2 a = d == 0 ? make_float2(0.f, 0.f) : accum[(pos << CS) + col];
+                a.x += c * v.y;   // times -i kt_d: (re, im) -> (kt im, -kt re)
+                a.y -= c * v.x;
+                if (d == 2) {
+                    const float G = mode_green(g, pos, iy, iz);
+                    a.x *= G;
+                    a.y *= G;
+                }
+                accum[(pos << CS) + col] = a;
+            }
+        }
+        __syncthreads();
+    }
+    AxisFFT<NX, NX, true, B, CS>::run(accum, ncol, tw);
+    tile_store<NX, CS>(accum, psi + off, stride, ncol);
+}
+
+// ---- z pass, real -> half-complex, in place on ZROWS consecutive z-rows per CTA ---------------------------------
+// row = [zs floats] -> [zsc complex]; x_n real, n < Nz = 2M: z_n = x_2n + i x_2n+1, Z = FFT_M(z),
+// E_k = (Z_k + conj Z_{M-k}) / 2, O_k = (Z_k - conj Z_{M-k}) / (2i), X_k = E_k + w^k O_k, w = e^{-2 pi i / Nz}, k = 0..M
+// shared: tile [M][ZP] + out [M + 1][ZP] + M twiddles + (M + 1) post twiddles + M positions
+template <int M>
+__global__ void __launch_bounds__(FFT_T) fft_z_r2c_kernel(FftGeom g, float *data, long long nrows)
+{
+    extern __shared__ __align__(16) unsigned char fsm[];
+    float2 *tile = reinterpret_cast<float2 *>(fsm);
+    float2 *outb = tile + M * ZP;
+    float2 *tw = outb + (M + 1) * ZP;
+    float2 *twr = tw + M;
+    int *posz = reinterpret_cast<int *>(twr + (M + 1));
+    const int zs = 2 * g.zsc;
+    const long long row0 = (long long)blockIdx.x * ZROWS;
+    const int nr = (int)min((long long)ZROWS, nrows - row0);
+    float *rows = data + (size_t)row0 * zs;
+    // thread -> (row, pair index) with the pair index fastest: coalesced 8-byte loads
+    constexpr int RPP = FFT_T / M > 0 ? FFT_T / M : 1;   // rows per pass when M <= FFT_T
+    if (M <= FFT_T) {
+        const int n = threadIdx.x % M, r0 = threadIdx.x / M;
+#pragma unroll 4
+        for (int r = r0; r < nr; r += RPP) tile[n * ZP + r] = *reinterpret_cast<const float2 *>(rows + (size_t)r * zs + 2 * n);
+    } else {
+        for (int r = 0; r < nr; r++)
+            for (int n = threadIdx.x; n < M; n += FFT_T) tile[n * ZP + r] = *reinterpret_cast<const float2 *>(rows + (size_t)r * zs + 2 * n);
+    }
+    load_tw(tw, g.twz, M);
+    load_tw(twr, g.twzr, M + 1);
+    for (int i = threadIdx.x; i < M; i += FFT_T) posz[i] = g.posz[i];
+    __syncthreads();
+    AxisFFT<M, M, false, ZP, 4>::run(tile, nr, tw);
+    {
+        const int r = threadIdx.x & (ZROWS - 1);
+        if (r < nr) {
+#pragma unroll 4
+            for (int k = threadIdx.x >> 4; k <= M; k += FFT_T >> 4) {
+                const int km = k == M ? 0 : k, kc = (k == 0 || k == M) ? 0 : M - k;
+                const float2 a = tile[posz[km] * ZP + r], b = tile[posz[kc] * ZP + r];
+                const float2 E = make_float2(0.5f * (a.x + b.x), 0.5f * (a.y - b.y));
+                const float2 O = make_float2(0.5f * (a.y + b.y), -0.5f * (a.x - b.x));  // (a - conj b) / (2i)
+                outb[k * ZP + r] = cadd(E, cmul(twr[k], O));
+            }
+        }
+    }
+    __syncthreads();
+    float2 *crow = reinterpret_cast<float2 *>(rows);
+    for (int r = threadIdx.x / 64; r < nr; r += FFT_T / 64)
+        for (int k = threadIdx.x & 63; k < g.zsc; k += 64) crow[(size_t)r * g.zsc + k] = k <= M ? outb[k * ZP + r] : make_float2(0.f, 0.f);
+}
+
+// ---- z pass, half-complex -> real (unnormalised: Nz times the inverse), in place ------------------------------
+// E_k = X_k + conj X_{M-k}, O_k = (X_k - conj X_{M-k}) conj(w^k), Z_k = E_k + i O_k (twice the textbook Z: the
+// M-point inverse then yields Nz * x), z = IFFT_M(Z), x_2n = Re z_n, x_2n+1 = Im z_n
+template <int M>
+__global__ void __launch_bounds__(FFT_T) fft_z_c2r_kernel(FftGeom g, float *data, long long nrows)
+{
+    extern __shared__ __align__(16) unsigned char fsm[];
+    float2 *tile = reinterpret_cast<float2 *>(fsm);
+    float2 *inb = tile + M * ZP;
+    float2 *tw = inb + (M + 1) * ZP;
+    float2 *twr = tw + M;
+    int *posz = reinterpret_cast<int *>(twr + (M + 1));
+    const int zs = 2 * g.zsc;
+    const long long row0 = (long long)blockIdx.x * ZROWS;
+    const int nr = (int)min((long long)ZROWS, nrows - row0);
+    float *rows = data + (size_t)row0 * zs;
+    const float2 *crow = reinterpret_cast<const float2 *>(rows);
+    for (int r = threadIdx.x / 64; r < nr; r += FFT_T / 64)
+        for (int k = threadIdx.x & 63; k <= M; k += 64) inb[k * ZP + r] = crow[(size_t)r * g.zsc + k];
+    load_tw(tw, g.twz, M);
+    load_tw(twr, g.twzr, M + 1);
+    for (int i = threadIdx.x; i < M; i += FFT_T) posz[i] = g.posz[i];
+    __syncthreads();
+    {
+        const int r = threadIdx.x & (ZROWS - 1);
+        if (r < nr) {
+#pragma unroll 4
+            for (int k = threadIdx.x >> 4; k < M; k += FFT_T >> 4) {
+                const float2 a = inb[k * ZP + r], b = inb[(M - k) * ZP + r];
+                const float2 E = make_float2(a.x + b.x, a.y - b.y);
+                const float2 O = cmulc(make_float2(a.x - b.x, a.y + b.y), twr[k]);
+                tile[posz[k] * ZP + r] = make_float2(E.x - O.y, E.y + O.x);  // E + i O
+            }
+        }
+    }
+    __syncthreads();
+    AxisFFT<M, M, true, ZP, 4>::run(tile, nr, tw);
+    if (M <= FFT_T) {
+        constexpr int RPP = FFT_T / M > 0 ? FFT_T / M : 1;
+        const int n = threadIdx.x % M, r0 = threadIdx.x / M;
+#pragma unroll 4
+        for (int r = r0; r < nr; r += RPP) *reinterpret_cast<float2 *>(rows + (size_t)r * zs + 2 * n) = tile[n * ZP + r];
+    } else {
+        for (int r = 0; r < nr; r++)
+            for (int n = threadIdx.x; n < M; n += FFT_T) *reinterpret_cast<float2 *>(rows + (size_t)r * zs + 2 * n) = tile[n * ZP + r];
+    }
+}
+
+// ---- host ------------------------------------------------------------------------------------------------------
+static bool is_pow2(int v) { return v > 0 && (v & (v - 1)) == 0; }
+
+static AxisPlan make_axis_plan(int N)
+{
+    AxisPlan p;
+    p.N = N;
+    p.nst = 0;
+    int n = N;
+    while (n > 1) {
+        int r = n >= 16 ? 16 : n;  // 16, ..., then the remainder 8 / 4 / 2
+        p.radix[p.nst] = r;
+        p.span[p.nst] = n;
+        p.nst++;
+        n /= r;
+    }
+    return p;
+}
+
+// frequency held at memory position pos after the forward stages of the plan
+static int freq_of_pos(const AxisPlan &p, int pos)
+{
+    int k = 0, mul = 1, L = p.N;
+    for (int s = 0; s < p.nst; s++) {
+        int Lr = L / p.radix[s];
+        int q = pos / Lr;
+        k += q * mul;
+        mul *= p.radix[s];
+        pos -= q * Lr;
+        L = Lr;
+    }
+    return k;
+}
+
+bool fft_own_supported(const Geometry &g)
+{
+    const char *e = getenv("PM_FFT");
+    if (e && strcmp(e, "cufft") == 0) return false;
+    for (int d = 0; d < 3; d++)
+        if (!is_pow2(g.N[d]) || g.N[d] < 16 || g.N[d] > 1024) return false;
+    return true;
+}
+
+size_t fft_own_table_bytes(const Geometry &g)
+{
+    return sizeof(float2) * (size_t)(g.N[0] + g.N[1] + g.N[2] + 16) + sizeof(int) * (size_t)g.N[2] + 1024;
+}
+
+// memory order of an axis in k-space: the frequency index (0..N-1, cuFFT order) stored at each position
+void fft_own_axis_order(const pm_ctx *c, int axis, std::vector<int> &freq)
+{
+    const int N = c->g.N[axis];
+    freq.resize(N);
+    if (!c->own_fft || axis == 2) {
+        for (int i = 0; i < N; i++) freq[i] = i;
+    } else {
+        AxisPlan p = make_axis_plan(N);
+        for (int i = 0; i < N; i++) freq[i] = freq_of_pos(p, i);
+    }
+}
+
+static FftGeom *geom_of(pm_ctx *c) { return reinterpret_cast<FftGeom *>(c->fft_geom); }
+
+int fft_own_init(pm_ctx *c)
+{
+    static_assert(sizeof(FftGeom) <= sizeof(c->fft_geom), "fft_geom storage too small");
+    const Geometry &g = c->g;
+    c->own_fft = fft_own_supported(g);
+    if (!c->own_fft) return PM_OK;
+    FftGeom *fg = geom_of(c);
+    const int M = g.N[2] / 2;
+    for (int d = 0; d < 3; d++) fg->N[d] = g.N[d];
+    fg->zsc = g.zs / 2;
+    fg->cstride = g.mesh_stride / 2;
+    const AxisPlan pz = make_axis_plan(M);
+    const double PI = 3.14159265358979323846264338327950288;
+    std::vector<float2> h;
+    auto push_tw = [&](int N, int count) {
+        size_t o = h.size();
+        for (int k = 0; k < count; k++) {
+            double a = -2.0 * PI * (double)k / (double)N;
+            h.push_back(make_float2((float)std::cos(a), (float)std::sin(a)));
+        }
+        return o;
+    };
+    size_t ox = push_tw(g.N[0], g.N[0]), oy = push_tw(g.N[1], g.N[1]), oz = push_tw(M, M), ozr = push_tw(g.N[2], M + 1);
+    std::vector<int> posz(M);
+    for (int pos = 0; pos < M; pos++) posz[freq_of_pos(pz, pos)] = pos;
+    float2 *dtab = reinterpret_cast<float2 *>(c->fft_tab);
+    int *dpos = reinterpret_cast<int *>(dtab + ((h.size() + 15) / 16) * 16);
+    PM_CUDA(c, cudaMemcpy(dtab, h.data(), sizeof(float2) * h.size(), cudaMemcpyHostToDevice));
+    PM_CUDA(c, cudaMemcpy(dpos, posz.data(), sizeof(int) * posz.size(), cudaMemcpyHostToDevice));
+    fg->twx = dtab + ox;
+    fg->twy = dtab + oy;
+    fg->twz = dtab + oz;
+    fg->twzr = dtab + ozr;
+    fg->posz = dpos;
+    fg->ktab = c->ktab;
+    fg->tabn = c->ktabn;
+    fg->c0 = 0.0;
+    return PM_OK;
+}
+
+#define PM_FFT_LAUNCH(ctx, name, kernel, grid, smem, ...)                                  \
+    do {                                                                                   \
+        static size_t attr_ = 0;                                                           \
+        if ((smem) > attr_) {                                                              \
+            PM_CUDA(ctx, cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(smem))); \
+            attr_ = (smem);                                                                \
+        }                                                                                  \
+        kernel<<<grid, FFT_T, smem, (ctx)->stream>>>(__VA_ARGS__);                         \
+        PM_LAUNCH_CHECK(ctx, name);                                                        \
+    } while (0)
+
+// N is a template parameter of every kernel: dispatch over the supported powers of two
+#define PM_FFT_SWITCH(n, CASE)          \
+    switch (n) {                        \
+        case 8: CASE(8, 4); break;      \
+        case 16: CASE(16, 4); break;    \
+        case 32: CASE(32, 4); break;    \
+        case 64: CASE(64, 4); break;    \
+        case 128: CASE(128, 4); break;  \
+        case 256: CASE(256, 4); break;  \
+        case 512: CASE(512, 3); break;  \
+        case 1024: CASE(1024, 3); break; \
+        default: return fail(c, PM_EINVAL, "own FFT", "unsupported axis length"); \
+    }
+
+static int fft_z(pm_ctx *c, float *mesh, int nb, bool inverse)
+{
+    const Geometry &g = c->g;
+    FftGeom fg = *geom_of(c);
+    const int M = g.N[2] / 2;
+    long long nrows = (long long)nb * g.N[0] * g.N[1];
+    unsigned grid = (unsigned)((nrows + ZROWS - 1) / ZROWS);
+    size_t smem = sizeof(float2) * ((size_t)M * ZP + (size_t)(M + 1) * ZP + M + (M + 1)) + sizeof(int) * (size_t)M;
+    Timer t(c, inverse ? TC_FFT_Z_C2R : TC_FFT_Z_R2C, 8.0 * (double)g.ng * nb);
+#define Z_CASE(NN, CS_)                                                                                     \
+    if (inverse) PM_FFT_LAUNCH(c, "fft_z_c2r_kernel", fft_z_c2r_kernel<NN>, grid, smem, fg, mesh, nrows);  \
+    else PM_FFT_LAUNCH(c, "fft_z_r2c_kernel", fft_z_r2c_kernel<NN>, grid, smem, fg, mesh, nrows)
+    switch (M) {
+        case 8: Z_CASE(8, 4); break;
+        case 16: Z_CASE(16, 4); break;
+        case 32: Z_CASE(32, 4); break;
+        case 64: Z_CASE(64, 4); break;
+        case 128: Z_CASE(128, 4); break;
+        case 256: Z_CASE(256, 4); break;
+        case 512: Z_CASE(512, 4); break;
+        default: return fail(c, PM_EINVAL, "own FFT", "unsupported Nz");
+    }
+#undef Z_CASE
+    t.stop();
+    return PM_OK;
+}
+
+static int fft_y(pm_ctx *c, float *mesh, int nb, bool inverse)
+{
+    const Geometry &g = c->g;
+    FftGeom fg = *geom_of(c);
+    const int cs = g.N[1] <= 256 ? 4 : 3, B = 1 << cs;
+    dim3 grid((unsigned)((fg.zsc + B - 1) / B), (unsigned)g.N[0], (unsigned)nb);
+    size_t smem = sizeof(float2) * ((size_t)g.N[1] + (size_t)g.N[1] * B);
+    Timer t(c, TC_FFT_Y, 16.0 * (double)g.nk * nb);
+#define Y_CASE(NN, CS_)                                                                                                   \
+    if (inverse) PM_FFT_LAUNCH(c, "fft_y_kernel<inv>", (fft_y_kernel<NN, CS_, true>), grid, smem, fg, (float2 *)mesh);   \
+    else PM_FFT_LAUNCH(c, "fft_y_kernel<fwd>", (fft_y_kernel<NN, CS_, false>), grid, smem, fg, (float2 *)mesh)
+    PM_FFT_SWITCH(g.N[1], Y_CASE)
+#undef Y_CASE
+    t.stop();
+    return PM_OK;
+}
+
+static int fft_x_fused(pm_ctx *c, const float *in, float *out, double nbar, bool adjoint)
+{
+    const Geometry &g = c->g;
+    FftGeom fg = *geom_of(c);
+    fg.c0 = 1.5 * c->prm.omega_m / (nbar * (double)g.ng);
+    const int cs = g.N[0] <= 256 ? 4 : 3, B = 1 << cs;
+    dim3 grid((unsigned)((fg.zsc + B - 1) / B), (unsigned)g.N[1]);
+    size_t smem = sizeof(float2) * ((size_t)g.N[0] + 2 * (size_t)g.N[0] * B) + sizeof(float) * (size_t)g.N[0];
+    Timer t(c, adjoint ? TC_KSPACE_ADJ : TC_KSPACE_FORCE, 32.0 * (double)g.nk);
+#define X_CASE(NN, CS_)                                                                                                                   \
+    if (adjoint) PM_FFT_LAUNCH(c, "fft_x_adjoint_kernel", (fft_x_adjoint_kernel<NN, CS_>), grid, smem, fg, (const float2 *)in, (float2 *)out); \
+    else PM_FFT_LAUNCH(c, "fft_x_force_kernel", (fft_x_force_kernel<NN, CS_>), grid, smem, fg, (const float2 *)in, (float2 *)out)
+    PM_FFT_SWITCH(g.N[0], X_CASE)
+#undef X_CASE
+    t.stop();
+    return PM_OK;
+}
+
+// rho (1 mesh, real, padded) -> f_d (3 meshes, real, padded): eq. 11 with the spectral gradient (L127-131)
+int fft_own_force(pm_ctx *c, float *rho, float *f3, double nbar)
+{
+    PM_TRY(fft_z(c, rho, 1, false));
+    PM_TRY(fft_y(c, rho, 1, false));
+    PM_TRY(fft_x_fused(c, rho, f3, nbar, false));
+    PM_TRY(fft_y(c, f3, 3, true));
+    PM_TRY(fft_z(c, f3, 3, true));
+    return PM_OK;
+}
+
+// Pi_d (3 meshes) -> psi (1 mesh): the transpose of the force operator
+int fft_own_adjoint(pm_ctx *c, float *Pi3, float *psi, double nbar)
+{
+    PM_TRY(fft_z(c, Pi3, 3, false));
+    PM_TRY(fft_y(c, Pi3, 3, false));
+    PM_TRY(fft_x_fused(c, Pi3, psi, nbar, true));
+    PM_TRY(fft_y(c, psi, 1, true));
+    PM_TRY(fft_z(c, psi, 1, true));
+    return PM_OK;
+}
+
+}  // namespace pm

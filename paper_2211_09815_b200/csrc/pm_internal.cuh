@@ -36,6 +36,9 @@ enum TimingClass {
     TC_KSPACE_ADJ,
     TC_FFT_R2C,
     TC_FFT_C2R,
+    TC_FFT_Z_R2C,
+    TC_FFT_Z_C2R,
+    TC_FFT_Y,
     TC_KICK_DRIFT,
     TC_OBJECTIVE,
     TC_CONVERT,
@@ -96,6 +99,9 @@ struct pm_ctx {
     CUtensorMap tmap_load, tmap_store;  // 4-D {z, y, x, mesh 0..6} views of the internal meshes: halo box / tile box
     bool tma_ok;                 // cuTensorMapEncodeTiled resolved and the internal maps encoded
     void *fft_work;
+    bool own_fft;                // power-of-two mesh: own FFT passes with the k-space operators fused (pm_fft.cu)
+    void *fft_tab;               // twiddle / position tables of the own FFT
+    alignas(8) unsigned char fft_geom[320];  // pm::FftGeom (pm_fft.cu)
     size_t fft_work_bytes;
     // integrator bookkeeping
     int t_index;                 // state is at t_{t_index}; -1 = no state
@@ -170,6 +176,14 @@ int gather_fused_sorted(pm_ctx *c, const float *mesh4, int zs, long long ms, con
 // ---- k-space (pm_kspace.cu) -------------------------------------------------------------------------
 int kspace_force(pm_ctx *c, const float2 *rho_k, float2 *f_k /*3 meshes, stride ms/2*/, double nbar);
 int kspace_adjoint(pm_ctx *c, const float2 *Pi_k /*3 meshes*/, float2 *psi_k, double nbar);
+
+// ---- own FFT with fused k-space operators (pm_fft.cu) ------------------------------------------------
+bool fft_own_supported(const Geometry &g);
+size_t fft_own_table_bytes(const Geometry &g);
+int fft_own_init(pm_ctx *c);                                  // needs c->ktab, c->fft_tab carved
+void fft_own_axis_order(const pm_ctx *c, int axis, std::vector<int> &freq);  // frequency index stored at each memory position
+int fft_own_force(pm_ctx *c, float *rho, float *f3, double nbar);
+int fft_own_adjoint(pm_ctx *c, float *Pi3, float *psi, double nbar);
 
 // ---- integrator elementwise kernels (pm_integrate.cu) -----------------------------------------------
 int state_from_float(pm_ctx *c, const float *s, const float *p);
