@@ -254,20 +254,34 @@ __global__ void __launch_bounds__(FFT_T) fft_x_force_kernel(FftGeom g, const flo
         }
     }
     // (no barrier needed: every thread re-reads only the elements it has just written)
-#pragma unroll 1
-    for (int d = 0; d < 3; d++) {
-        if (col < ncol) {
+    // kt_y and kt_z do not depend on x, so ONE inverse transform of G rho serves f_y and f_z; f_x needs its own
+    if (col < ncol) {
 #pragma unroll 4
-            for (int pos = threadIdx.x >> CS; pos < NX; pos += FFT_T >> CS) {
-                const float c = d == 0 ? ktx[pos] : (d == 1 ? kty : ktz);
-                const float2 r = spec[(pos << CS) + col];
-                work[(pos << CS) + col] = make_float2(-c * r.y, c * r.x);  // times +i kt_d
+        for (int pos = threadIdx.x >> CS; pos < NX; pos += FFT_T >> CS) {
+            const float c = ktx[pos];
+            const float2 r = spec[(pos << CS) + col];
+            work[(pos << CS) + col] = make_float2(-c * r.y, c * r.x);  // times +i kt_x
+        }
+    }
+    __syncthreads();
+    AxisFFT<NX, NX, true, B, CS>::run(work, ncol, tw);
+    tile_store<NX, CS>(work, f + off, stride, ncol);
+    AxisFFT<NX, NX, true, B, CS>::run(spec, ncol, tw);
+    // f_y = i kt_y T, f_z = i kt_z T with T = the back-transformed G rho; 16-byte stores of column pairs
+    {
+        constexpr int HB = 1 << (CS - 1);
+        const int cp = threadIdx.x & (HB - 1);
+        if (2 * cp < ncol) {
+            const float kz0 = (float)g.ktab[6 * g.tabn + min(col0 + 2 * cp, g.N[2] / 2)];
+            const float kz1 = (float)g.ktab[6 * g.tabn + min(col0 + 2 * cp + 1, g.N[2] / 2)];
+#pragma unroll 4
+            for (int pos = threadIdx.x >> (CS - 1); pos < NX; pos += FFT_T >> (CS - 1)) {
+                const float4 t4 = *reinterpret_cast<const float4 *>(spec + (pos << CS) + 2 * cp);
+                float2 *dst = f + g.cstride + off + (size_t)pos * stride + 2 * cp;
+                *reinterpret_cast<float4 *>(dst) = make_float4(-kty * t4.y, kty * t4.x, -kty * t4.w, kty * t4.z);
+                *reinterpret_cast<float4 *>(dst + g.cstride) = make_float4(-kz0 * t4.y, kz0 * t4.x, -kz1 * t4.w, kz1 * t4.z);
             }
         }
-        __syncthreads();
-        AxisFFT<NX, NX, true, B, CS>::run(work, ncol, tw);
-        tile_store<NX, CS>(work, f + (size_t)d * g.cstride + off, stride, ncol);
-        __syncthreads();
     }
 }
 
@@ -290,30 +304,36 @@ __global__ void __launch_bounds__(FFT_T) fft_x_adjoint_kernel(FftGeom g, const f
     const float kty = (float)g.ktab[3 * g.tabn + iy], ktz = (float)g.ktab[6 * g.tabn + iz];
     load_tw(tw, g.twx, NX);
     for (int i = threadIdx.x; i < NX; i += FFT_T) ktx[i] = (float)g.ktab[i];
-#pragma unroll 1
-    for (int d = 0; d < 3; d++) {
-        tile_load<NX, CS>(work, Pi + (size_t)d * g.cstride + off, stride, ncol);
-        fft_cp_async_wait_all();
-        __syncthreads();
-        AxisFFT<NX, NX, false, B, CS>::run(work, ncol, tw);
-        if (col < ncol) {
+    // kt_y and kt_z do not depend on x: kt_y Pi_y + kt_z Pi_z is formed BEFORE the transform along x, so two forward
+    // transforms (Pi_x and that sum) instead of three
+    tile_load<NX, CS>(accum, Pi + g.cstride + off, stride, ncol);
+    tile_load<NX, CS>(work, Pi + 2 * g.cstride + off, stride, ncol);
+    fft_cp_async_wait_all();
+    __syncthreads();
+    if (col < ncol) {
 #pragma unroll 4
-            for (int pos = threadIdx.x >> CS; pos < NX; pos += FFT_T >> CS) {
-                const float c = d == 0 ? ktx[pos] : (d == 1 ? kty : ktz);
-                const float2 v = work[(pos << CS) + col];
-                float2 a = d == 0 ? make_float2(0.f, 0.f) : accum[(pos << CS) + col];
-                a.x += c * v.y;   // times -i kt_d: (re, im) -> (kt im, -kt re)
-                a.y -= c * v.x;
-                if (d == 2) {
-                    const float G = mode_green(g, pos, iy, iz);
-                    a.x *= G;
-                    a.y *= G;
-                }
-                accum[(pos << CS) + col] = a;
-            }
+        for (int pos = threadIdx.x >> CS; pos < NX; pos += FFT_T >> CS) {
+            const float2 vy = accum[(pos << CS) + col], vz = work[(pos << CS) + col];
+            accum[(pos << CS) + col] = make_float2(kty * vy.x + ktz * vz.x, kty * vy.y + ktz * vz.y);
         }
-        __syncthreads();
     }
+    __syncthreads();
+    tile_load<NX, CS>(work, Pi + off, stride, ncol);
+    AxisFFT<NX, NX, false, B, CS>::run(accum, ncol, tw);
+    fft_cp_async_wait_all();
+    __syncthreads();
+    AxisFFT<NX, NX, false, B, CS>::run(work, ncol, tw);
+    if (col < ncol) {
+#pragma unroll 4
+        for (int pos = threadIdx.x >> CS; pos < NX; pos += FFT_T >> CS) {
+            const float c = ktx[pos];
+            const float2 v = work[(pos << CS) + col], a = accum[(pos << CS) + col];
+            const float G = mode_green(g, pos, iy, iz);
+            // times -i G: (re, im) -> (G im, -G re)
+            accum[(pos << CS) + col] = make_float2(G * (c * v.y + a.y), -G * (c * v.x + a.x));
+        }
+    }
+    __syncthreads();
     AxisFFT<NX, NX, true, B, CS>::run(accum, ncol, tw);
     tile_store<NX, CS>(accum, psi + off, stride, ncol);
 }
@@ -328,28 +348,35 @@ __global__ void __launch_bounds__(FFT_T) fft_z_r2c_kernel(FftGeom g, float *data
     extern __shared__ __align__(16) unsigned char fsm[];
     float2 *tile = reinterpret_cast<float2 *>(fsm);
     float2 *outb = tile + M * ZP;
-    float2 *tw = outb + (M + 1) * ZP;
+    float2 *tw = outb + max((M + 1) * ZP, ZROWS * g.zsc);
     float2 *twr = tw + M;
     int *posz = reinterpret_cast<int *>(twr + (M + 1));
     const int zs = 2 * g.zsc;
     const long long row0 = (long long)blockIdx.x * ZROWS;
     const int nr = (int)min((long long)ZROWS, nrows - row0);
     float *rows = data + (size_t)row0 * zs;
-    // thread -> (row, pair index) with the pair index fastest: coalesced 8-byte loads
-    constexpr int RPP = FFT_T / M > 0 ? FFT_T / M : 1;   // rows per pass when M <= FFT_T
-    if (M <= FFT_T) {
-        const int n = threadIdx.x % M, r0 = threadIdx.x / M;
-#pragma unroll 4
-        for (int r = r0; r < nr; r += RPP) tile[n * ZP + r] = *reinterpret_cast<const float2 *>(rows + (size_t)r * zs + 2 * n);
-    } else {
-        for (int r = 0; r < nr; r++)
-            for (int n = threadIdx.x; n < M; n += FFT_T) tile[n * ZP + r] = *reinterpret_cast<const float2 *>(rows + (size_t)r * zs + 2 * n);
+    // the nr rows are contiguous in memory: 16-byte async copies into a row-major staging area (which shares its
+    // shared memory with outb), then the transposing fill of the tile
+    float *stage = reinterpret_cast<float *>(outb);
+    {
+        const int nchunk = nr * (zs / 4);
+        for (int i = threadIdx.x; i < nchunk; i += FFT_T) fft_cp_async16(stage + 4 * i, rows + 4 * (size_t)i);
     }
     load_tw(tw, g.twz, M);
     load_tw(twr, g.twzr, M + 1);
     for (int i = threadIdx.x; i < M; i += FFT_T) posz[i] = g.posz[i];
+    fft_cp_async_wait_all();
+    __syncthreads();
+    {
+        const int r = threadIdx.x & (ZROWS - 1);
+        if (r < nr) {
+#pragma unroll 4
+            for (int n = threadIdx.x >> 4; n < M; n += FFT_T >> 4) tile[n * ZP + r] = *reinterpret_cast<const float2 *>(stage + r * zs + 2 * n);
+        }
+    }
     __syncthreads();
     AxisFFT<M, M, false, ZP, 4>::run(tile, nr, tw);
+
     {
         const int r = threadIdx.x & (ZROWS - 1);
         if (r < nr) {
@@ -378,26 +405,28 @@ __global__ void __launch_bounds__(FFT_T) fft_z_c2r_kernel(FftGeom g, float *data
     extern __shared__ __align__(16) unsigned char fsm[];
     float2 *tile = reinterpret_cast<float2 *>(fsm);
     float2 *inb = tile + M * ZP;
-    float2 *tw = inb + (M + 1) * ZP;
+    float2 *tw = inb + max((M + 1) * ZP, ZROWS * g.zsc);
     float2 *twr = tw + M;
     int *posz = reinterpret_cast<int *>(twr + (M + 1));
     const int zs = 2 * g.zsc;
     const long long row0 = (long long)blockIdx.x * ZROWS;
     const int nr = (int)min((long long)ZROWS, nrows - row0);
     float *rows = data + (size_t)row0 * zs;
-    const float2 *crow = reinterpret_cast<const float2 *>(rows);
-    for (int r = threadIdx.x / 64; r < nr; r += FFT_T / 64)
-        for (int k = threadIdx.x & 63; k <= M; k += 64) inb[k * ZP + r] = crow[(size_t)r * g.zsc + k];
+    {   // the nr rows are contiguous in memory: 16-byte async copies, row-major [row][zsc]
+        const int nchunk = nr * (zs / 4);
+        for (int i = threadIdx.x; i < nchunk; i += FFT_T) fft_cp_async16(reinterpret_cast<float *>(inb) + 4 * i, rows + 4 * (size_t)i);
+    }
     load_tw(tw, g.twz, M);
     load_tw(twr, g.twzr, M + 1);
     for (int i = threadIdx.x; i < M; i += FFT_T) posz[i] = g.posz[i];
+    fft_cp_async_wait_all();
     __syncthreads();
     {
         const int r = threadIdx.x & (ZROWS - 1);
         if (r < nr) {
 #pragma unroll 4
             for (int k = threadIdx.x >> 4; k < M; k += FFT_T >> 4) {
-                const float2 a = inb[k * ZP + r], b = inb[(M - k) * ZP + r];
+                const float2 a = inb[r * g.zsc + k], b = inb[r * g.zsc + M - k];
                 const float2 E = make_float2(a.x + b.x, a.y - b.y);
                 const float2 O = cmulc(make_float2(a.x - b.x, a.y + b.y), twr[k]);
                 tile[posz[k] * ZP + r] = make_float2(E.x - O.y, E.y + O.x);  // E + i O
@@ -552,7 +581,9 @@ static int fft_z(pm_ctx *c, float *mesh, int nb, bool inverse)
     const int M = g.N[2] / 2;
     long long nrows = (long long)nb * g.N[0] * g.N[1];
     unsigned grid = (unsigned)((nrows + ZROWS - 1) / ZROWS);
-    size_t smem = sizeof(float2) * ((size_t)M * ZP + (size_t)(M + 1) * ZP + M + (M + 1)) + sizeof(int) * (size_t)M;
+    size_t second = (size_t)(M + 1) * ZP;                       // outb / inb: transposed [M + 1][ZP] or row-major staging
+    if (second < (size_t)ZROWS * (g.zs / 2)) second = (size_t)ZROWS * (g.zs / 2);
+    size_t smem = sizeof(float2) * ((size_t)M * ZP + second + M + (M + 1)) + sizeof(int) * (size_t)M;
     Timer t(c, inverse ? TC_FFT_Z_C2R : TC_FFT_Z_R2C, 8.0 * (double)g.ng * nb);
 #define Z_CASE(NN, CS_)                                                                                     \
     if (inverse) PM_FFT_LAUNCH(c, "fft_z_c2r_kernel", fft_z_c2r_kernel<NN>, grid, smem, fg, mesh, nrows);  \
