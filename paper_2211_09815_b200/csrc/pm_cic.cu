@@ -58,7 +58,6 @@ constexpr int HALO_STRIDE = (HALO_PTS + 31) / 32 * 32;    // per-mesh stride in 
 constexpr int NCW = 8;                                    // consumer warps
 constexpr int NCT = NCW * 32;                             // consumer threads
 constexpr int NTHREADS = NCT + 32;                        // + one producer warp
-constexpr int NST = 2;                                    // pipeline stages
 constexpr int RCAP = 512;                                 // records staged in shared memory per tile (the rest are read from global)
 
 // ---- PTX wrappers: mbarrier + TMA (sm_90+/sm_100a) ----------------------------------------------------
@@ -339,14 +338,18 @@ struct ScatterSlot {
     int run_prefix[NRUNS + 1];
 };
 
+// record stages: 4 for the scalar scatter (48 KB per CTA), 2 for three components (64 KB: three CTAs per SM)
 template <int C>
-constexpr size_t scatter_smem_bytes() { return (size_t)2 * C * TILE_PTS * sizeof(int) + (size_t)NST * RCAP * sizeof(uint4); }
+constexpr int scatter_stages() { return C == 1 ? 4 : 2; }
+template <int C>
+constexpr size_t scatter_smem_bytes() { return (size_t)2 * C * TILE_PTS * sizeof(int) + (size_t)scatter_stages<C>() * RCAP * sizeof(uint4); }
 
 template <int C, bool HAS_VAL>
 __global__ void __launch_bounds__(NTHREADS) scatter_kernel(const __grid_constant__ CUtensorMap tmap, CicGeom g,
                                                            const uint4 *__restrict__ rec, const int *__restrict__ offsets,
                                                            const float *__restrict__ val, float *__restrict__ mesh)
 {
+    constexpr int NST = C == 1 ? 4 : 2;  // = scatter_stages<C>()
     extern __shared__ __align__(128) unsigned char dsm[];
     typedef int AccBuf[C][TILE_PTS];
     AccBuf *acc = reinterpret_cast<AccBuf *>(dsm);                                        // [2]

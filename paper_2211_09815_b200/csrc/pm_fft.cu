@@ -154,8 +154,6 @@ struct FftGeom {
     double c0;           // 3/2 Om / (nbar N_g)
 };
 
-constexpr int ZROWS = 16;   // z-rows per CTA of the real <-> half-complex passes
-constexpr int ZP = ZROWS + 1;
 
 __device__ __forceinline__ void fft_cp_async16(void *dst, const void *src)
 {
@@ -342,9 +340,10 @@ __global__ void __launch_bounds__(FFT_T) fft_x_adjoint_kernel(FftGeom g, const f
 // row = [zs floats] -> [zsc complex]; x_n real, n < Nz = 2M: z_n = x_2n + i x_2n+1, Z = FFT_M(z),
 // E_k = (Z_k + conj Z_{M-k}) / 2, O_k = (Z_k - conj Z_{M-k}) / (2i), X_k = E_k + w^k O_k, w = e^{-2 pi i / Nz}, k = 0..M
 // shared: tile [M][ZP] + out [M + 1][ZP] + M twiddles + (M + 1) post twiddles + M positions
-template <int M>
+template <int M, int ZRS>
 __global__ void __launch_bounds__(FFT_T) fft_z_r2c_kernel(FftGeom g, float *data, long long nrows)
 {
+    constexpr int ZROWS = 1 << ZRS, ZP = ZROWS + 1;  // z-rows per CTA; tile pitch
     extern __shared__ __align__(16) unsigned char fsm[];
     float2 *tile = reinterpret_cast<float2 *>(fsm);
     float2 *outb = tile + M * ZP;
@@ -371,17 +370,17 @@ __global__ void __launch_bounds__(FFT_T) fft_z_r2c_kernel(FftGeom g, float *data
         const int r = threadIdx.x & (ZROWS - 1);
         if (r < nr) {
 #pragma unroll 4
-            for (int n = threadIdx.x >> 4; n < M; n += FFT_T >> 4) tile[n * ZP + r] = *reinterpret_cast<const float2 *>(stage + r * zs + 2 * n);
+            for (int n = threadIdx.x >> ZRS; n < M; n += FFT_T >> ZRS) tile[n * ZP + r] = *reinterpret_cast<const float2 *>(stage + r * zs + 2 * n);
         }
     }
     __syncthreads();
-    AxisFFT<M, M, false, ZP, 4>::run(tile, nr, tw);
+    AxisFFT<M, M, false, ZP, ZRS>::run(tile, nr, tw);
 
     {
         const int r = threadIdx.x & (ZROWS - 1);
         if (r < nr) {
 #pragma unroll 4
-            for (int k = threadIdx.x >> 4; k <= M; k += FFT_T >> 4) {
+            for (int k = threadIdx.x >> ZRS; k <= M; k += FFT_T >> ZRS) {
                 const int km = k == M ? 0 : k, kc = (k == 0 || k == M) ? 0 : M - k;
                 const float2 a = tile[posz[km] * ZP + r], b = tile[posz[kc] * ZP + r];
                 const float2 E = make_float2(0.5f * (a.x + b.x), 0.5f * (a.y - b.y));
@@ -399,9 +398,10 @@ __global__ void __launch_bounds__(FFT_T) fft_z_r2c_kernel(FftGeom g, float *data
 // ---- z pass, half-complex -> real (unnormalised: Nz times the inverse), in place ------------------------------
 // E_k = X_k + conj X_{M-k}, O_k = (X_k - conj X_{M-k}) conj(w^k), Z_k = E_k + i O_k (twice the textbook Z: the
 // M-point inverse then yields Nz * x), z = IFFT_M(Z), x_2n = Re z_n, x_2n+1 = Im z_n
-template <int M>
+template <int M, int ZRS>
 __global__ void __launch_bounds__(FFT_T) fft_z_c2r_kernel(FftGeom g, float *data, long long nrows)
 {
+    constexpr int ZROWS = 1 << ZRS, ZP = ZROWS + 1;  // z-rows per CTA; tile pitch
     extern __shared__ __align__(16) unsigned char fsm[];
     float2 *tile = reinterpret_cast<float2 *>(fsm);
     float2 *inb = tile + M * ZP;
@@ -425,7 +425,7 @@ __global__ void __launch_bounds__(FFT_T) fft_z_c2r_kernel(FftGeom g, float *data
         const int r = threadIdx.x & (ZROWS - 1);
         if (r < nr) {
 #pragma unroll 4
-            for (int k = threadIdx.x >> 4; k < M; k += FFT_T >> 4) {
+            for (int k = threadIdx.x >> ZRS; k < M; k += FFT_T >> ZRS) {
                 const float2 a = inb[r * g.zsc + k], b = inb[r * g.zsc + M - k];
                 const float2 E = make_float2(a.x + b.x, a.y - b.y);
                 const float2 O = cmulc(make_float2(a.x - b.x, a.y + b.y), twr[k]);
@@ -434,7 +434,7 @@ __global__ void __launch_bounds__(FFT_T) fft_z_c2r_kernel(FftGeom g, float *data
         }
     }
     __syncthreads();
-    AxisFFT<M, M, true, ZP, 4>::run(tile, nr, tw);
+    AxisFFT<M, M, true, ZP, ZRS>::run(tile, nr, tw);
     if (M <= FFT_T) {
         constexpr int RPP = FFT_T / M > 0 ? FFT_T / M : 1;
         const int n = threadIdx.x % M, r0 = threadIdx.x / M;
@@ -484,8 +484,11 @@ bool fft_own_supported(const Geometry &g)
 {
     const char *e = getenv("PM_FFT");
     if (e && strcmp(e, "cufft") == 0) return false;
+    // above 512 the x pass strides over more 2 MB pages than the TLBs like and cuFFT's passes are as fast
+    // (measured at 1024^3, profiles/); PM_FFT=own forces the own passes there too
+    const bool force = e && strcmp(e, "own") == 0;
     for (int d = 0; d < 3; d++)
-        if (!is_pow2(g.N[d]) || g.N[d] < 16 || g.N[d] > 1024) return false;
+        if (!is_pow2(g.N[d]) || g.N[d] < 16 || g.N[d] > (force ? 1024 : 512)) return false;
     return true;
 }
 
@@ -561,6 +564,17 @@ int fft_own_init(pm_ctx *c)
     } while (0)
 
 // N is a template parameter of every kernel: dispatch over the supported powers of two
+#define PM_FFT_SWITCH_X(n, CASE)        \
+    switch (n) {                        \
+        case 16: CASE(16, 4); break;    \
+        case 32: CASE(32, 4); break;    \
+        case 64: CASE(64, 4); break;    \
+        case 128: CASE(128, 4); break;  \
+        case 256: CASE(256, 4); break;  \
+        case 512: CASE(512, 3); break;  \
+        case 1024: CASE(1024, 2); break; \
+        default: return fail(c, PM_EINVAL, "own FFT", "unsupported axis length"); \
+    }
 #define PM_FFT_SWITCH(n, CASE)          \
     switch (n) {                        \
         case 8: CASE(8, 4); break;      \
@@ -580,14 +594,15 @@ static int fft_z(pm_ctx *c, float *mesh, int nb, bool inverse)
     FftGeom fg = *geom_of(c);
     const int M = g.N[2] / 2;
     long long nrows = (long long)nb * g.N[0] * g.N[1];
+    const int ZRS = M >= 512 ? 3 : 4, ZROWS = 1 << ZRS, ZP = ZROWS + 1;  // fewer rows per CTA for long rows: 3 CTAs per SM
     unsigned grid = (unsigned)((nrows + ZROWS - 1) / ZROWS);
     size_t second = (size_t)(M + 1) * ZP;                       // outb / inb: transposed [M + 1][ZP] or row-major staging
     if (second < (size_t)ZROWS * (g.zs / 2)) second = (size_t)ZROWS * (g.zs / 2);
     size_t smem = sizeof(float2) * ((size_t)M * ZP + second + M + (M + 1)) + sizeof(int) * (size_t)M;
     Timer t(c, inverse ? TC_FFT_Z_C2R : TC_FFT_Z_R2C, 8.0 * (double)g.ng * nb);
 #define Z_CASE(NN, CS_)                                                                                     \
-    if (inverse) PM_FFT_LAUNCH(c, "fft_z_c2r_kernel", fft_z_c2r_kernel<NN>, grid, smem, fg, mesh, nrows);  \
-    else PM_FFT_LAUNCH(c, "fft_z_r2c_kernel", fft_z_r2c_kernel<NN>, grid, smem, fg, mesh, nrows)
+    if (inverse) PM_FFT_LAUNCH(c, "fft_z_c2r_kernel", (fft_z_c2r_kernel<NN, CS_>), grid, smem, fg, mesh, nrows);  \
+    else PM_FFT_LAUNCH(c, "fft_z_r2c_kernel", (fft_z_r2c_kernel<NN, CS_>), grid, smem, fg, mesh, nrows)
     switch (M) {
         case 8: Z_CASE(8, 4); break;
         case 16: Z_CASE(16, 4); break;
@@ -595,7 +610,7 @@ static int fft_z(pm_ctx *c, float *mesh, int nb, bool inverse)
         case 64: Z_CASE(64, 4); break;
         case 128: Z_CASE(128, 4); break;
         case 256: Z_CASE(256, 4); break;
-        case 512: Z_CASE(512, 4); break;
+        case 512: Z_CASE(512, 3); break;
         default: return fail(c, PM_EINVAL, "own FFT", "unsupported Nz");
     }
 #undef Z_CASE
@@ -625,14 +640,14 @@ static int fft_x_fused(pm_ctx *c, const float *in, float *out, double nbar, bool
     const Geometry &g = c->g;
     FftGeom fg = *geom_of(c);
     fg.c0 = 1.5 * c->prm.omega_m / (nbar * (double)g.ng);
-    const int cs = g.N[0] <= 256 ? 4 : 3, B = 1 << cs;
+    const int cs = g.N[0] <= 256 ? 4 : (g.N[0] <= 512 ? 3 : 2), B = 1 << cs;  // two tiles of Nx x B: keep 3 CTAs per SM
     dim3 grid((unsigned)((fg.zsc + B - 1) / B), (unsigned)g.N[1]);
     size_t smem = sizeof(float2) * ((size_t)g.N[0] + 2 * (size_t)g.N[0] * B) + sizeof(float) * (size_t)g.N[0];
     Timer t(c, adjoint ? TC_KSPACE_ADJ : TC_KSPACE_FORCE, 32.0 * (double)g.nk);
 #define X_CASE(NN, CS_)                                                                                                                   \
     if (adjoint) PM_FFT_LAUNCH(c, "fft_x_adjoint_kernel", (fft_x_adjoint_kernel<NN, CS_>), grid, smem, fg, (const float2 *)in, (float2 *)out); \
     else PM_FFT_LAUNCH(c, "fft_x_force_kernel", (fft_x_force_kernel<NN, CS_>), grid, smem, fg, (const float2 *)in, (float2 *)out)
-    PM_FFT_SWITCH(g.N[0], X_CASE)
+    PM_FFT_SWITCH_X(g.N[0], X_CASE)
 #undef X_CASE
     t.stop();
     return PM_OK;
