@@ -170,20 +170,28 @@ def run_ours(args):
     def step_dev():
         J[0] = pm.run_fwd_adj(s0d, p0d, tgd, out=outs)["J"]
 
-    # ---- device-resident timing (value): per-kernel CUDA events on libpm's stream are live here ----
+    # ---- device-resident timing (value): K steps, nothing but the run in the timed region ----
     for _ in range(args.warmup):
         step_dev()
     own0, fft0 = pm.launch_count()
-    pm.timing_enable(True)
-    pm.timing_reset()
     clocks = ClockSampler(local)
     ms = timed(step_dev, args.steps)
     clk = clocks.stop()
     own1, fft1 = pm.launch_count()
-    tm = pm.timing_read()
-    pm.timing_enable(False)
-    pm.timing_reset()
     value = world * npart * n * args.steps / (ms * 1e-3)
+
+    # ---- the same K steps again with a CUDA-event pair around every launch (recorded by libpm on its own stream):
+    #      per-kernel durations for the roofline and the kernel table.  The events cost a few per cent of the step
+    #      (ms_per_step_instrumented), which is why `value` is not taken from this pass. ----
+    tm = {}
+    ms_instr = None
+    if not args.no_kernel_timing:
+        pm.timing_enable(True)
+        pm.timing_reset()
+        ms_instr = timed(step_dev, args.steps)
+        tm = pm.timing_read()
+        pm.timing_enable(False)
+        pm.timing_reset()
 
     # ---- end to end through host buffers (e2e): H2D of inputs and D2H of results inside the timed region ----
     hin = [torch.from_numpy(v).pin_memory() for v in (s0, p0, target)]
@@ -208,17 +216,23 @@ def run_ours(args):
             gbs = v["algo_bytes"] / v["launches"] / (per_ms * 1e-3) / 1e9
             kernels[name] = {"launches_per_step": v["launches"] / args.steps, "avg_ms": per_ms, "share": v["ms"] / tot_ms,
                              "algo_GBps": gbs, "frac_of_peak": gbs / peak}
-    own = {k: v for k, v in kernels.items() if not k.startswith("fft_")}
+    own = {k: v for k, v in kernels.items() if k not in ("fft_r2c", "fft_c2r")}  # cuFFT calls are listed, not graded
+    if not own:  # --no-kernel-timing
+        own = {"none": {"share": 0.0, "algo_GBps": 0.0}}
     dom = max(own, key=lambda k: own[k]["share"])
-    traffic = None
+    traffic = None  # DRAM bytes per launch of that kernel from the committed ncu --set full capture (profiles/), or null
     try:
-        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
-            traffic = json.load(f).get(cfg["name"], {}).get(dom)
+        with open(os.path.join(ROOT, "profiles", "r01b_traffic.csv")) as f:
+            for ln in f:
+                parts = ln.strip().split(",")
+                if len(parts) == 3 and parts[0] == cfg["name"] and parts[1] == dom:
+                    traffic = float(parts[2])
     except Exception:
         pass
     roofline = {"bound": "hbm", "kernel": dom, "achieved": own[dom]["algo_GBps"], "peak": peak, "unit": "GB/s",
                 "frac": own[dom]["algo_GBps"] / peak, "traffic": traffic, "peak_source": peak_src,
-                "share_of_step": own[dom]["share"]}
+                "share_of_step": own[dom]["share"],
+                "timing": "CUDA events around every launch on the library's stream, second pass of the same K steps"}
 
     line = None
     if rank == 0:
@@ -231,6 +245,7 @@ def run_ours(args):
                 "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                         "ms_per_step": ms_h / args.steps},
                 "gpu_launches": int(own1 - own0), "cufft_calls": int(fft1 - fft0),
+                "ms_per_step_instrumented": None if ms_instr is None else ms_instr / args.steps,
                 "clocks": clk, "roofline": roofline, "kernels": kernels, "objective_J": J[0],
                 "peak_mem_GB": torch.cuda.max_memory_allocated() / 1e9}
         if world == 1 and not args.no_cpu_baseline:
@@ -244,18 +259,81 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_sweep(args):
+    """configs[4]: CIC scatter / gather / weight-gradient gather of 512^3 particles on a 1024^3 mesh, clustered
+    (20000 Gaussian blobs, 70 % of the particles) against uniform positions, in generation and in random memory
+    order; GB/s = SURVEY section 8d algorithmic bytes / CUDA-event time, with and without the binning pass."""
+    import torch
+    from paper_2211_09815_b200 import binding
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(0)
+    L = args.sweep_lattice
+    N = 2 * L
+    mesh, npart = (N, N, N), L ** 3
+    pm = binding.PM(mesh, (L, L, L), 0.3, [1.0])
+    peak, peak_src = measured_peak_gbs()
+    gen = torch.Generator(device="cuda").manual_seed(5)
+    f3 = torch.randn((3,) + mesh, device="cuda", generator=gen)
+    val = torch.randn((npart, 3), device="cuda", generator=gen)
+    ng = float(N) ** 3
+    algo = {"scatter1": 12.0 * npart + 4.0 * ng, "scatter3": 24.0 * npart + 12.0 * ng, "gather3": 24.0 * npart + 12.0 * ng,
+            "gather_grad1": 24.0 * npart + 4.0 * ng}
+    ops = {"scatter1": lambda x: pm.scatter(x), "scatter3": lambda x: pm.scatter(x, val), "gather3": lambda x: pm.gather(x, f3),
+           "gather_grad1": lambda x: pm.gather_grad(x, f3[0])}
+    cls_of = {"scatter1": "scatter1", "scatter3": "scatter3", "gather3": "gather", "gather_grad1": "gather_grad"}
+    n_blobs = max(1, int(round(20000 * npart / 512.0 ** 3)))
+    cases = {"clustered/generation": lambda: inputs.blob_positions(npart, mesh, seed=3, n_blobs=n_blobs, order="generation"),
+             "clustered/random": lambda: inputs.blob_positions(npart, mesh, seed=3, n_blobs=n_blobs, order="random"),
+             "uniform/generation": lambda: inputs.uniform_positions(npart, mesh, seed=3)}
+    out = {}
+    for cname, make in cases.items():
+        x = torch.from_numpy(make()).cuda()
+        res = {}
+        for oname, op in ops.items():
+            for _ in range(max(args.warmup, 1)):
+                op(x)
+            torch.cuda.synchronize()
+            pm.timing_enable(True)
+            pm.timing_reset()
+            for _ in range(args.steps):
+                op(x)
+            torch.cuda.synchronize()
+            tm = pm.timing_read()
+            pm.timing_enable(False)
+            pm.timing_reset()
+            k_ms = tm[cls_of[oname]]["ms"] / args.steps
+            bin_ms = sum(tm[b]["ms"] for b in ("bin_count", "bin_scan", "bin_reorder")) / args.steps
+            res[oname] = {"kernel_ms": k_ms, "binning_ms": bin_ms, "GBps": algo[oname] / (k_ms * 1e-3) / 1e9,
+                          "frac_of_peak": algo[oname] / (k_ms * 1e-3) / 1e9 / peak,
+                          "GBps_with_binning": algo[oname] / ((k_ms + bin_ms) * 1e-3) / 1e9}
+        out[cname] = res
+        del x
+    line = {"metric": "CIC scatter/gather GB/s vs HBM peak (kernel sweep)", "value": out["clustered/generation"]["scatter1"]["GBps"],
+            "unit": "GB/s", "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "higher_is_better": True, "dtype": "f32",
+            "data": "synthetic", "vs_baseline": None,
+            "config": {"workload": f"cfg4_kernel_sweep_{L}p_{N}m", "particles": npart, "mesh": list(mesh), "blobs": n_blobs},
+            "peak": peak, "peak_source": peak_src, "sweep": out, "peak_mem_GB": torch.cuda.max_memory_allocated() / 1e9}
+    print(json.dumps(line), flush=True)
+    pm.close()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=1, help="BASELINE.json configs index (0-3)")
+    ap.add_argument("--config", type=int, default=1, help="BASELINE.json configs index (0-3; 4 = the CIC kernel sweep)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--ref-steps", type=int, default=1, help="KDK steps in the oracle's bounded sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-kernel-timing", action="store_true", help="no per-kernel CUDA events in the timed region (debug)")
+    ap.add_argument("--sweep-lattice", type=int, default=512, help="particles per axis of the configs[4] kernel sweep (mesh = 2x)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.config == 4:
+        run_sweep(args)
     else:
         run_ours(args)
 

@@ -234,3 +234,45 @@ def test_stepwise_calls_match_whole_run(pmlib, orc):
     assert torch.equal(s_n, whole["s_n"]) and torch.equal(p_n, whole["p_n"])
     assert torch.equal(xi, whole["xi0"]) and torch.equal(pi, whole["pi0"]) and torch.equal(g, whole["dJ_ds0"])
     pm.close()
+
+
+def test_own_fft_matches_cufft_path(pmlib, orc, monkeypatch):
+    """The power-of-two meshes take the library's own FFT passes with the k-space operators fused into the x pass
+    (csrc/pm_fft.cu); PM_FFT=cufft forces the cuFFT + separate k-space kernel path the other meshes use.  Two
+    independent implementations of eq. 11 (L127-131) and of its transpose on a non-cubic mesh whose three axes
+    exercise different radix plans (64 = 16 x 4, 128 = 16 x 8, Nz/2 = 128), and the oracle on a sample."""
+    mesh, lattice = (64, 128, 256), (32, 64, 128)
+    rng = np.random.default_rng(31)
+    npart = int(np.prod(lattice))
+    x = (rng.random((npart, 3)) * np.asarray(mesh)).astype(np.float32)
+    x[: npart // 8] = (np.asarray(mesh) * 0.61 + rng.normal(0, 1.5, (npart // 8, 3))).astype(np.float32)
+    pi = rng.standard_normal((npart, 3)).astype(np.float32)
+    res = {}
+    for mode in ("own", "cufft"):
+        monkeypatch.setenv("PM_FFT", mode)
+        pm = pmlib.PM(mesh, lattice, 0.3, [0.5, 1.0])
+        acc, alpha = pm.force_vjp(dev(x), dev(pi))
+        res[mode] = (acc.cpu().numpy(), alpha.cpu().numpy())
+        pm.close()
+    assert rel_l2(res["own"][0], res["cufft"][0]) <= 2e-6
+    assert rel_l2(res["own"][1], res["cufft"][1]) <= 2e-6
+    acc_o = orc.force(mesh, 0.3, x)
+    assert rel_l2(res["own"][0], acc_o) <= 1e-5
+    alpha_o = orc.force_vjp(mesh, 0.3, x, pi)
+    assert rel_l2(res["own"][1], alpha_o) <= 1e-5
+
+
+def test_valued_scatter_is_order_independent(pmlib):
+    """The scale of the valued scatter comes from integer atomics and a float max only (csrc/pm_cic.cu): permuting
+    the particles must not change a single bit, also with a dense clump and values spanning orders of magnitude."""
+    mesh, lattice = (48, 40, 64), (24, 20, 32)
+    rng = np.random.default_rng(6)
+    pm = pmlib.PM(mesh, lattice, 1.0, [0.5, 1.0])
+    x = rand_positions(rng, pm.np, mesh)
+    x[: pm.np // 4] = (np.asarray(mesh) * 0.37 + rng.normal(0, 0.4, (pm.np // 4, 3))).astype(np.float32)
+    val = (rng.standard_normal((pm.np, 3)) * np.exp(rng.normal(0, 2, (pm.np, 1)))).astype(np.float32)
+    a = pm.scatter(dev(x), dev(val)).cpu().numpy()
+    perm = rng.permutation(pm.np)
+    b = pm.scatter(dev(x[perm]), dev(val[perm])).cpu().numpy()
+    assert np.array_equal(a, b)
+    pm.close()
