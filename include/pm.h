@@ -1,7 +1,8 @@
 /*
  * pm.h -- C ABI of libpm: the data-parallel hot path of the adjoint particle-mesh method of
  * "Differentiable Cosmological Simulation with the Adjoint Method" (arxiv 2211.09815),
- * hand-written CUDA for sm_100a (B200).  cuFFT is used for the 3-D transforms only.
+ * hand-written CUDA for sm_100a (B200).  The 3-D transforms are the library's own passes on power-of-two
+ * meshes up to 512 per axis (k-space operators fused in) and cuFFT's on every other mesh.
  *
  * Citations are /root/reference/PAPER.md line numbers (L..) with the equation they fall in.
  *
@@ -35,7 +36,7 @@ typedef struct pm_ctx pm_ctx; /* opaque, host memory owned by the library */
 
 typedef struct {
     int32_t mesh[3];     /* Nx, Ny, Nz mesh points per axis; each >= 2, Nz even; each <= 4096       */
-    int32_t lattice[3];  /* particle lattice Lx, Ly, Lz; N_p = product; (mesh[d] << fbits) % lattice[d] == 0
+    int32_t lattice[3];  /* particle lattice Lx, Ly, Lz; N_p = product; (mesh[d] << 32) % lattice[d] == 0
                             (true whenever lattice divides mesh, the case of every config)            */
     double omega_m;      /* flat matter + Lambda: Omega_Lambda = 1 - omega_m; 1.0 = Einstein-de Sitter */
     int32_t n_steps;     /* n >= 0 KDK steps                                                           */
@@ -103,7 +104,7 @@ int pm_force_vjp(pm_ctx *ctx, int64_t np, const float *dev_x, const float *dev_p
 /* ---- state-carrying reversible integrator (eq. 16; eq. 49-50) ------------------------
  * The state (s, p, acc) and the adjoint variables (xi, pi, alpha) live inside the workspace; s and p
  * are held in fixed point so that every kick and drift is undone EXACTLY by the reverse pass
- * (DESIGN.md "Reversibility").  Displacements must stay below 2^(31-fbits) cells in magnitude.       */
+ * (DESIGN.md "Reversibility"): absolute position int64 at 2^-32 cell, momentum int64 at 2^-36.       */
 
 /* copy in s0, p0 [N_p][3] (displacement in cells, canonical momentum p = a^2 dx/dt in cells*H0),
  * set the time index to 0 and compute acc_0 = F(q + s_0) (L175) */
