@@ -93,9 +93,10 @@ __device__ __forceinline__ void mbar_arrive(unsigned long long *bar)
 }
 __device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned phase)
 {
+    // try_wait with a suspend-time hint: a waiting warp sleeps in hardware instead of spinning through the issue slots
     asm volatile(
-        "{\n .reg .pred p;\n WAIT_%=:\n mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n @p bra DONE_%=;\n bra WAIT_%=;\n DONE_%=:\n}"
-        ::"r"(smem_u32(bar)), "r"(phase)
+        "{\n .reg .pred p;\n WAIT_%=:\n mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n @p bra DONE_%=;\n bra WAIT_%=;\n DONE_%=:\n}"
+        ::"r"(smem_u32(bar)), "r"(phase), "r"(20000u)
         : "memory");
 }
 __device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *m, unsigned long long *bar, int z, int y, int x, int c)
@@ -661,9 +662,14 @@ struct GatherSlot {
     int beg, end;
 };
 
-constexpr int GST = 2;                                     // halo stages per CTA: GST - 1 tiles in flight while one is computed
+// halo stages per CTA (GST - 1 tiles in flight while one is computed).  Measured at 256^3: a single 47 KB stage for the
+// four-mesh fused gather (three CTAs per SM instead of two) is slower (230 vs 221 us), three stages are slower too.
+#define PM_GST(C) ((C) == 4 ? PM_GST4 : 2)
+#ifndef PM_GST4
+#define PM_GST4 2
+#endif
 template <int C>
-constexpr size_t gather_smem_bytes() { return (size_t)GST * C * HALO_STRIDE * sizeof(float); }
+constexpr size_t gather_smem_bytes() { return (size_t)PM_GST(C) * C * HALO_STRIDE * sizeof(float); }
 
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N>
@@ -761,6 +767,8 @@ __global__ void __launch_bounds__(GT) gather_kernel(CicGeom g, const uint4 *__re
                                                     const float *__restrict__ mesh, const float *cot, float cot_scale,
                                                     float *__restrict__ out, float *__restrict__ out2, PosGeom pg, KickArgs ka)
 {
+    constexpr int GST = PM_GST(C);
+    constexpr int PUB = GST < 2 ? 2 : GST;  // tiles are published PUB iterations ahead (the record prefetch looks one ahead)
     extern __shared__ __align__(128) unsigned char dsm[];
     __shared__ GatherSlot slot[8];  // ring of drawn tiles: iteration n computes slot[n & 7] and starts the copies of slot[(n + GST - 1) & 7]
     auto halo_of = [&](int s) { return reinterpret_cast<float *>(dsm) + (size_t)s * C * HALO_STRIDE; };
@@ -787,7 +795,7 @@ __global__ void __launch_bounds__(GT) gather_kernel(CicGeom g, const uint4 *__re
     if (tid == 0) {
         d_atom = atomicAdd(&g.sched[0], 1);
         draw_request();
-        for (int k = 0; k < GST; k++) {
+        for (int k = 0; k < PUB; k++) {
             draw_publish(slot[k]);
             draw_request();
         }
@@ -923,10 +931,10 @@ __global__ void __launch_bounds__(GT) gather_kernel(CicGeom g, const uint4 *__re
         q = q_nx;
         if (has_nx) pin.load(q.w, cot, ka);
         if (tid == 0) {
-            draw_publish(slot[(n + GST) & 7]);
+            draw_publish(slot[(n + PUB) & 7]);
             draw_request();
         }
-        __syncthreads();  // stage n % GST may be overwritten; slot[(n + GST) & 7] is published
+        __syncthreads();  // stage n % GST may be overwritten; slot[(n + PUB) & 7] is published
     }
     cp_async_wait<0>();
     if (tid == 0) sched_finish(g.sched);
