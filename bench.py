@@ -73,6 +73,22 @@ class ClockSampler:
                 "reasons": reasons, "samples": len(sm)}
 
 
+def max_over_ranks(ms, world, device):
+    """Replicas: the job's time is the slowest rank's device time."""
+    if world <= 1:
+        return float(ms)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_value(world, npart, n_steps, runs, ms):
+    """Whole-job particle-steps/s: every rank runs its own replica of the same size, no data-path collective."""
+    return world * npart * n_steps * runs / (ms * 1e-3)
+
+
 def measured_peak_gbs():
     try:
         with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
@@ -158,12 +174,7 @@ def run_ours(args):
             fn()
         e1.record(stream)
         barrier()
-        ms = e0.elapsed_time(e1)
-        if world > 1:
-            t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
-        return ms
+        return max_over_ranks(e0.elapsed_time(e1), world, "cuda")
 
     J = [0.0]
 
@@ -178,7 +189,7 @@ def run_ours(args):
     ms = timed(step_dev, args.steps)
     clk = clocks.stop()
     own1, fft1 = pm.launch_count()
-    value = world * npart * n * args.steps / (ms * 1e-3)
+    value = job_value(world, npart, n, args.steps, ms)
 
     # ---- the same K steps again with a CUDA-event pair around every launch (recorded by libpm on its own stream):
     #      per-kernel durations for the roofline and the kernel table.  The events cost a few per cent of the step
@@ -202,7 +213,7 @@ def run_ours(args):
 
     step_host()
     ms_h = timed(step_host, args.steps)
-    e2e = world * npart * n * args.steps / (ms_h * 1e-3)
+    e2e = job_value(world, npart, n, args.steps, ms_h)
     h2d = sum(t.numel() * 4 for t in hin)
     d2h = sum(t.numel() * 4 for t in hout.values()) + 8
 
