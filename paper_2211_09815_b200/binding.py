@@ -13,6 +13,17 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libpm.so")
 
 if not os.path.exists(LIB_PATH):
+    # a fresh checkout on a box with nvcc: compile once (under a lock, ranks may import concurrently); never a fallback
+    try:
+        import fcntl
+        from . import build as _build
+        with open(os.path.join(_HERE, ".build.lock"), "w") as _lk:
+            fcntl.flock(_lk, fcntl.LOCK_EX)
+            if not os.path.exists(LIB_PATH):
+                _build.build(force=True)
+    except Exception:  # noqa: BLE001  (reported just below)
+        pass
+if not os.path.exists(LIB_PATH):
     raise ImportError(
         f"{LIB_PATH} is missing: build it with `python -m paper_2211_09815_b200.build` "
         "(nvcc, sm_100a). There is no CPU fallback.")

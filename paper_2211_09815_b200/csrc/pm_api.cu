@@ -76,7 +76,7 @@ static int make_geometry(const pm_params *p, Geometry *g, const char **why)
         }
     }
     int fb = 32 - ceil_log2(maxn);
-    g->fbits = fb > 22 ? 22 : fb;
+    g->fbits = fb > 24 ? 24 : fb;  // <= 24: the fraction and 1 - fraction stay exact in fp32
     g->np = 1;
     g->ng = 1;
     for (int d = 0; d < 3; d++) {

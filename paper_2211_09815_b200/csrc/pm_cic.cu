@@ -337,6 +337,10 @@ struct ScatterSlot {
     int n0;                     // leading records of the tile's own class 0 (all corners inside)
     int run_start[NRUNS];       // rec index = run_start[r] + flat index
     int run_prefix[NRUNS + 1];
+    int t0[3], ext[3];          // first mesh point and extent of the tile (computed once, by the producer)
+    float scale, inv_scale;     // unit-mass fixed-point scale of the tile
+    float mrest;                // mean subtraction: sub-quantum rest ...
+    long long mq;               // ... and whole quanta
 };
 
 // record stages: 4 for the scalar scatter (48 KB per CTA), 2 for three components (64 KB: three CTAs per SM)
@@ -436,6 +440,30 @@ __global__ void __launch_bounds__(NTHREADS) scatter_kernel(const __grid_constant
                 slot[s].tile = tile;
                 slot[s].total = total;
                 slot[s].n0 = n0;
+                {
+                    int tt[3], tt0[3], text[3];
+                    tile_coords(g, tile, tt, tt0, text);
+#pragma unroll
+                    for (int d = 0; d < 3; d++) { slot[s].t0[d] = tt0[d]; slot[s].ext[d] = text[d]; }
+                    // unit mass: deposits are >= 0 -> UNSIGNED accumulation with scale = (2^32 - headroom) / total.  total is
+                    // an integer, so the scale is the same in every run: the density mesh stays bit-reproducible.  No point
+                    // can overflow: sum of weights at a point <= total, and each of the <= total deposits rounds by <= 0.5.
+                    const float room = fmaxf(4294967296.f * 0.99999f - (float)total, 1.f);
+                    const float sc = ldexpf(room / fmaxf((float)total, 1.f), -g.kshift);
+                    const float isc = 1.f / sc;
+                    slot[s].scale = sc;
+                    slot[s].inv_scale = isc;
+                    // mean subtraction (unit mass): mq quanta are removed exactly in integer, the sub-quantum rest in fp32
+                    long long mq = 0;
+                    float mrest = 0.f;
+                    if (g.mean != 0.0) {
+                        const double m = g.mean * (double)sc;
+                        mq = __double2ll_rn(m);
+                        mrest = (float)((m - (double)mq) * (double)isc);
+                    }
+                    slot[s].mq = mq;
+                    slot[s].mrest = mrest;
+                }
                 // the tile's own run: one bulk copy; the (short) neighbour runs: 16-byte async copies, one lane per run
                 if (cnt > 0) {
                     mbar_expect_tx(&full[s], (unsigned)cnt * (unsigned)sizeof(uint4));
@@ -469,8 +497,7 @@ __global__ void __launch_bounds__(NTHREADS) scatter_kernel(const __grid_constant
         const int tile = sl.tile;
         if (tile < 0) break;
         const int total = sl.total, n0 = sl.n0;
-        int t[3], t0[3], ext[3];
-        tile_coords(g, tile, t, t0, ext);
+        const int t0[3] = {sl.t0[0], sl.t0[1], sl.t0[2]}, ext[3] = {sl.ext[0], sl.ext[1], sl.ext[2]};
 
         // flat index -> record: the first RCAP are staged in shared memory, the rest come from global
         auto fetch = [&](int i) -> uint4 {
@@ -487,11 +514,7 @@ __global__ void __launch_bounds__(NTHREADS) scatter_kernel(const __grid_constant
 
         float scale;
         if (!HAS_VAL) {
-            // unit mass: deposits are >= 0 -> UNSIGNED accumulation with scale = (2^32 - headroom) / total.  total is an
-            // integer, so the scale is the same in every run: the density mesh stays bit-reproducible.  No point can
-            // overflow: sum of weights at a point <= total, and each of the <= total deposits rounds by <= 0.5.
-            const float room = fmaxf(4294967296.f * 0.99999f - (float)total, 1.f);
-            scale = ldexpf(room / fmaxf((float)total, 1.f), -g.kshift);
+            scale = sl.scale;  // unit mass: computed by the producer (see there)
             for (int i = tid; i < total; i += NCT) {
                 const uint4 q = fetch(i);
                 if (i < n0) {
@@ -586,15 +609,9 @@ __global__ void __launch_bounds__(NTHREADS) scatter_kernel(const __grid_constant
                 }
             }
         }
-        const float inv_scale = 1.f / scale;
-        // mean subtraction (unit mass): mq quanta are removed exactly in integer, the sub-quantum rest in fp32
-        long long mq = 0;
-        float mrest = 0.f;
-        if (!HAS_VAL && g.mean != 0.0) {
-            const double m = g.mean * (double)scale;
-            mq = __double2ll_rn(m);
-            mrest = (float)((m - (double)mq) * (double)inv_scale);
-        }
+        const float inv_scale = HAS_VAL ? 1.f / scale : sl.inv_scale;
+        const long long mq = HAS_VAL ? 0ll : sl.mq;
+        const float mrest = HAS_VAL ? 0.f : sl.mrest;
 
         if (tid == 0) tma_store_wait_read();  // the previous tile's store has read the other buffer out
         consumer_sync();                      // all deposits of this tile are in; the other buffer is free
@@ -660,6 +677,7 @@ constexpr int GRG = GT / GCH;                              // halo rows covered 
 struct GatherSlot {
     int tile;  // -1: no more tiles
     int beg, end;
+    int t0[3], ext[3];  // first mesh point and extent of the tile (computed once, by the drawing thread)
 };
 
 // halo stages per CTA (GST - 1 tiles in flight while one is computed).  Measured at 256^3: a single 47 KB stage for the
@@ -677,10 +695,9 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 
 // starts the copies of one tile's halo (C meshes) into `halo`; every thread of the CTA takes part
 template <int C>
-__device__ __forceinline__ void halo_issue(const CicGeom &g, const float *__restrict__ mesh, int tile, float *halo)
+__device__ __forceinline__ void halo_issue(const CicGeom &g, const float *__restrict__ mesh, const GatherSlot &sl, float *halo)
 {
-    int t[3], t0[3], ext[3];
-    tile_coords(g, tile, t, t0, ext);
+    const int t0[3] = {sl.t0[0], sl.t0[1], sl.t0[2]}, ext[3] = {sl.ext[0], sl.ext[1], sl.ext[2]};
     const bool rows_ok = g.use_tma && (g.N[2] & 3) == 0;  // 16-byte aligned rows
     if (rows_ok) {
         // rows (lx, ly), lx <= ext[0], ly <= ext[1], wrapped periodically; along z either HZP contiguous floats or,
@@ -693,8 +710,9 @@ __device__ __forceinline__ void halo_issue(const CicGeom &g, const float *__rest
         const int rg = threadIdx.x / GCH, ch = threadIdx.x - rg * GCH;
         if (rg < GRG && ch < cpr) {
             const int zoff = ch < cpr_main ? t0[2] + ch * 4 : 0;
-            int lx = rg / ny, ly = rg - lx * ny;
-            const int dlx = GRG / ny, dly = GRG - dlx * ny;
+            // full tiles (ny == HY): compile-time divisors
+            int lx = ny == HY ? rg / HY : rg / ny, ly = rg - lx * ny;
+            const int dlx = ny == HY ? GRG / HY : GRG / ny, dly = GRG - dlx * ny;
             for (int r = rg; r < nrow; r += GRG) {
                 int gx = t0[0] + lx, gy = t0[1] + ly;
                 if (gx >= g.N[0]) gx -= g.N[0];
@@ -791,6 +809,12 @@ __global__ void __launch_bounds__(GT) gather_kernel(CicGeom g, const uint4 *__re
         dst.tile = d_tile < g.ntiles ? d_tile : -1;
         dst.beg = d_beg;
         dst.end = d_end;
+        if (d_tile < g.ntiles) {
+            int tt[3], tt0[3], text[3];
+            tile_coords(g, d_tile, tt, tt0, text);
+#pragma unroll
+            for (int d = 0; d < 3; d++) { dst.t0[d] = tt0[d]; dst.ext[d] = text[d]; }
+        }
     };
     if (tid == 0) {
         d_atom = atomicAdd(&g.sched[0], 1);
@@ -802,7 +826,7 @@ __global__ void __launch_bounds__(GT) gather_kernel(CicGeom g, const uint4 *__re
     }
     __syncthreads();
     for (int k = 0; k < GST - 1; k++) {
-        if (slot[k].tile >= 0 && slot[k].beg < slot[k].end) halo_issue<C>(g, mesh, slot[k].tile, halo_of(k));
+        if (slot[k].tile >= 0 && slot[k].beg < slot[k].end) halo_issue<C>(g, mesh, slot[k], halo_of(k));
         cp_async_commit();
     }
     // first round of the first tile: record and per-particle inputs
@@ -823,7 +847,7 @@ __global__ void __launch_bounds__(GT) gather_kernel(CicGeom g, const uint4 *__re
         // ended iteration n - 1)
         {
             const GatherSlot far = slot[(n + GST - 1) & 7];
-            if (far.tile >= 0 && far.beg < far.end && !(g.dbg & 2)) halo_issue<C>(g, mesh, far.tile, halo_of((n + GST - 1) % GST));
+            if (far.tile >= 0 && far.beg < far.end && !(g.dbg & 2)) halo_issue<C>(g, mesh, far, halo_of((n + GST - 1) % GST));
         }
         cp_async_commit();
         uint4 q_nx = make_uint4(0, 0, 0, 0);
@@ -832,8 +856,7 @@ __global__ void __launch_bounds__(GT) gather_kernel(CicGeom g, const uint4 *__re
         cp_async_wait<GST - 1>();  // this thread's copies of the current tile have landed ...
         __syncthreads();     // ... and everybody else's
 
-        int t[3], t0[3], ext[3];
-        tile_coords(g, cur.tile, t, t0, ext);
+        const int t0[3] = {cur.t0[0], cur.t0[1], cur.t0[2]};
         const float *halo = halo_of(n % GST);
         const int cnt = (g.dbg & 1) ? 0 : cur.end - cur.beg;
         for (int i = tid; i < cnt; i += GT) {
