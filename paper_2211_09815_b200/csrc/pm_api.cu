@@ -2,6 +2,7 @@
 // sequencing of the hot path (eq. 16 L172 forward; eq. 49-50 L393-397 adjoint; L400-408 run).
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -311,6 +312,17 @@ int pm_init(pm_ctx **out, const pm_params *params, void *dev_workspace, size_t b
     if (rc == PM_OK) rc = upload_ktab(c);
     if (rc == PM_OK) rc = fft_own_init(c);
     c->scan_epoch = 0;
+    c->overlap_ok = false;
+    {
+        const char *e = getenv("PM_OVERLAP");
+        if (!(e && atoi(e) == 0) && cudaStreamCreateWithFlags(&c->stream2, cudaStreamNonBlocking) == cudaSuccess) {
+            bool ok = cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) == cudaSuccess;
+            ok = ok && cudaEventCreateWithFlags(&c->ev_xforce, cudaEventDisableTiming) == cudaSuccess;
+            ok = ok && cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming) == cudaSuccess;
+            c->overlap_ok = ok;
+        }
+        (void)cudaGetLastError();
+    }
     {
         int dev = 0;
         c->num_sms = 148;
@@ -339,6 +351,12 @@ int pm_destroy(pm_ctx *c)
     }
     for (auto &r : c->trecs) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
     for (auto e : c->event_pool) cudaEventDestroy(e);
+    if (c->overlap_ok) {
+        cudaEventDestroy(c->ev_fork);
+        cudaEventDestroy(c->ev_xforce);
+        cudaEventDestroy(c->ev_join);
+        cudaStreamDestroy(c->stream2);
+    }
     delete c;
     return PM_OK;
 }

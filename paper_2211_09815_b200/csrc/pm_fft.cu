@@ -664,25 +664,35 @@ static int fft_x_fused(pm_ctx *c, const float *in, float *out, double nbar, bool
     return PM_OK;
 }
 
-// rho (1 mesh, real, padded) -> f_d (3 meshes, real, padded): eq. 11 with the spectral gradient (L127-131)
-int fft_own_force(pm_ctx *c, float *rho, float *f3, double nbar)
+// rho (1 mesh, real, padded) -> f_d (3 meshes, real, padded): eq. 11 with the spectral gradient (L127-131).
+// part 1 = z, y forward and the fused x kernel (rho is dead afterwards), part 2 = the inverse y and z passes; 0 = both
+int fft_own_force(pm_ctx *c, float *rho, float *f3, double nbar, int part)
 {
-    PM_TRY(fft_z(c, rho, 1, false));
-    PM_TRY(fft_y(c, rho, 1, false));
-    PM_TRY(fft_x_fused(c, rho, f3, nbar, false));
-    PM_TRY(fft_y(c, f3, 3, true));
-    PM_TRY(fft_z(c, f3, 3, true));
+    if (part != 2) {
+        PM_TRY(fft_z(c, rho, 1, false));
+        PM_TRY(fft_y(c, rho, 1, false));
+        PM_TRY(fft_x_fused(c, rho, f3, nbar, false));
+    }
+    if (part != 1) {
+        PM_TRY(fft_y(c, f3, 3, true));
+        PM_TRY(fft_z(c, f3, 3, true));
+    }
     return PM_OK;
 }
 
-// Pi_d (3 meshes) -> psi (1 mesh): the transpose of the force operator
-int fft_own_adjoint(pm_ctx *c, float *Pi3, float *psi, double nbar)
+// Pi_d (3 meshes) -> psi (1 mesh): the transpose of the force operator.
+// part 1 = z, y forward on the three meshes, part 2 = the fused x kernel (writes psi) and the inverse y, z; 0 = both
+int fft_own_adjoint(pm_ctx *c, float *Pi3, float *psi, double nbar, int part)
 {
-    PM_TRY(fft_z(c, Pi3, 3, false));
-    PM_TRY(fft_y(c, Pi3, 3, false));
-    PM_TRY(fft_x_fused(c, Pi3, psi, nbar, true));
-    PM_TRY(fft_y(c, psi, 1, true));
-    PM_TRY(fft_z(c, psi, 1, true));
+    if (part != 2) {
+        PM_TRY(fft_z(c, Pi3, 3, false));
+        PM_TRY(fft_y(c, Pi3, 3, false));
+    }
+    if (part != 1) {
+        PM_TRY(fft_x_fused(c, Pi3, psi, nbar, true));
+        PM_TRY(fft_y(c, psi, 1, true));
+        PM_TRY(fft_z(c, psi, 1, true));
+    }
     return PM_OK;
 }
 

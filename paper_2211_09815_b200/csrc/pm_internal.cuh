@@ -76,7 +76,10 @@ struct pm_ctx {
     std::vector<double> a;       // n+1 scale factors
     std::vector<double> fac;     // 3 per step: K1, D, K2 (forward)
     double p_over_s0;            // G_D(a0)/D1(a0)
-    cudaStream_t stream;
+    cudaStream_t stream;         // the stream launches go to (the caller's; temporarily stream2 inside StreamScope)
+    cudaStream_t stream2;        // second stream: the Pi branch of an adjoint step runs beside the force branch
+    cudaEvent_t ev_fork, ev_xforce, ev_join;
+    bool overlap_ok;             // stream2 and the events exist (and PM_OVERLAP != 0)
     cufftHandle plan_r2c1, plan_c2r1, plan_r2c3, plan_c2r3;
     bool plans_ok;
     // workspace carve-up (device pointers)
@@ -182,8 +185,8 @@ bool fft_own_supported(const Geometry &g);
 size_t fft_own_table_bytes(const Geometry &g);
 int fft_own_init(pm_ctx *c);                                  // needs c->ktab, c->fft_tab carved
 void fft_own_axis_order(const pm_ctx *c, int axis, std::vector<int> &freq);  // frequency index stored at each memory position
-int fft_own_force(pm_ctx *c, float *rho, float *f3, double nbar);
-int fft_own_adjoint(pm_ctx *c, float *Pi3, float *psi, double nbar);
+int fft_own_force(pm_ctx *c, float *rho, float *f3, double nbar, int part = 0);     // part: see pm_fft.cu
+int fft_own_adjoint(pm_ctx *c, float *Pi3, float *psi, double nbar, int part = 0);
 
 // ---- integrator elementwise kernels (pm_integrate.cu) -----------------------------------------------
 int state_from_float(pm_ctx *c, const float *s, const float *p);

@@ -276,3 +276,18 @@ def test_valued_scatter_is_order_independent(pmlib):
     b = pm.scatter(dev(x[perm]), dev(val[perm])).cpu().numpy()
     assert np.array_equal(a, b)
     pm.close()
+
+
+def test_two_stream_adjoint_step_is_bit_identical(pmlib, orc, monkeypatch):
+    """The adjoint step runs its force branch and its Pi branch on two streams (csrc/pm_api_ops.inc); PM_OVERLAP=0
+    keeps everything on one stream.  Same kernels, same arguments: every output must agree bit for bit."""
+    cfg, s0, p0, target = _cfg0_inputs(orc)
+    outs = {}
+    for mode in ("1", "0"):
+        monkeypatch.setenv("PM_OVERLAP", mode)
+        pm = pmlib.PM(cfg["mesh"], cfg["lattice"], cfg["omega_m"], cfg["a"])
+        outs[mode] = pm.run_fwd_adj(dev(s0), dev(p0), dev(target))
+        pm.close()
+    assert outs["1"]["J"] == outs["0"]["J"]
+    for k in ("s_n", "p_n", "xi0", "pi0", "dJ_ds0", "s_rec", "p_rec"):
+        assert torch.equal(outs["1"][k], outs["0"][k]), k
