@@ -220,13 +220,28 @@ __global__ void __launch_bounds__(FFT_T) fft_y_kernel(FftGeom g, float2 *data)
     tile_store<NY, CS>(tile, base, g.zsc, ncol);
 }
 
-// G(k) of one mode from the per-axis tables in memory order (fp64, rounded to fp32 once); G(0) = 0 (R9)
-__device__ __forceinline__ float mode_green(const FftGeom &g, int ix, int iy, int iz)
+// G(k) = c0 dec / k^2 of one mode, fp64 rounded to fp32 once; G(0) = 0 (R9).  The x-dependent table entries come from
+// shared memory, the (y, z)-dependent parts are per-thread constants; the division is a reciprocal seed refined by one
+// Newton step in fp64 (relative error ~1e-14, far below the final rounding to fp32).
+struct GreenCol {
+    double k2yz, decyz, c0;
+};
+__device__ __forceinline__ GreenCol green_col(const FftGeom &g, int iy, int iz)
 {
-    const double *tx = g.ktab, *ty = g.ktab + 3 * g.tabn, *tz = g.ktab + 6 * g.tabn;
-    const double k2 = tx[g.tabn + ix] + ty[g.tabn + iy] + tz[g.tabn + iz];
-    const double dec = tx[2 * g.tabn + ix] * ty[2 * g.tabn + iy] * tz[2 * g.tabn + iz];
-    return k2 > 0.0 ? (float)(g.c0 * dec / k2) : 0.f;
+    const double *ty = g.ktab + 3 * g.tabn, *tz = g.ktab + 6 * g.tabn;
+    GreenCol c;
+    c.k2yz = ty[g.tabn + iy] + tz[g.tabn + iz];
+    c.decyz = ty[2 * g.tabn + iy] * tz[2 * g.tabn + iz];
+    c.c0 = g.c0;
+    return c;
+}
+__device__ __forceinline__ float mode_green(const GreenCol &c, double k2x, double decx)
+{
+    const double k2 = k2x + c.k2yz;
+    if (!(k2 > 0.0)) return 0.f;
+    double r = (double)__frcp_rn((float)k2);
+    r = r * (2.0 - k2 * r);
+    return (float)(c.c0 * (decx * c.decyz) * r);
 }
 
 // ---- x pass fused with the force operator: rho(k) -> f_d(k) = i kt_d G rho(k), d = 1..3, back-transformed along x ----
@@ -239,14 +254,19 @@ __global__ void __launch_bounds__(FFT_T) fft_x_force_kernel(FftGeom g, const flo
     float2 *spec = reinterpret_cast<float2 *>(fsm);
     float2 *work = spec + (NX << CS);
     float2 *tw = work + (NX << CS);
-    float *ktx = reinterpret_cast<float *>(tw + NX);
+    double *k2x = reinterpret_cast<double *>(tw + NX), *decx = k2x + NX;
+    float *ktx = reinterpret_cast<float *>(decx + NX);
     const int col0 = blockIdx.x * B, ncol = min(B, g.zsc - col0);
     const int iy = blockIdx.y;
     const long long stride = (long long)g.N[1] * g.zsc;
     const size_t off = (size_t)iy * g.zsc + col0;
     tile_load<NX, CS>(spec, rho + off, stride, ncol);
     load_tw(tw, g.twx, NX);
-    for (int i = threadIdx.x; i < NX; i += FFT_T) ktx[i] = (float)g.ktab[i];
+    for (int i = threadIdx.x; i < NX; i += FFT_T) {
+        ktx[i] = (float)g.ktab[i];
+        k2x[i] = g.ktab[g.tabn + i];
+        decx[i] = g.ktab[2 * g.tabn + i];
+    }
     fft_cp_async_wait_all();
     __syncthreads();
     AxisFFT<NX, NX, false, B, CS>::run(spec, ncol, tw);
@@ -255,9 +275,10 @@ __global__ void __launch_bounds__(FFT_T) fft_x_force_kernel(FftGeom g, const flo
     const int iz = min(col0 + col, g.N[2] / 2);
     const float kty = (float)g.ktab[3 * g.tabn + iy], ktz = (float)g.ktab[6 * g.tabn + iz];
     if (col < ncol) {
+        const GreenCol gc = green_col(g, iy, iz);
 #pragma unroll 4
         for (int pos = threadIdx.x >> CS; pos < NX; pos += FFT_T >> CS) {
-            const float G = mode_green(g, pos, iy, iz);
+            const float G = mode_green(gc, k2x[pos], decx[pos]);
             float2 r = spec[(pos << CS) + col];
             spec[(pos << CS) + col] = make_float2(G * r.x, G * r.y);
         }
@@ -303,7 +324,8 @@ __global__ void __launch_bounds__(FFT_T) fft_x_adjoint_kernel(FftGeom g, const f
     float2 *accum = reinterpret_cast<float2 *>(fsm);
     float2 *work = accum + (NX << CS);
     float2 *tw = work + (NX << CS);
-    float *ktx = reinterpret_cast<float *>(tw + NX);
+    double *k2x = reinterpret_cast<double *>(tw + NX), *decx = k2x + NX;
+    float *ktx = reinterpret_cast<float *>(decx + NX);
     const int col0 = blockIdx.x * B, ncol = min(B, g.zsc - col0);
     const int iy = blockIdx.y;
     const long long stride = (long long)g.N[1] * g.zsc;
@@ -312,7 +334,11 @@ __global__ void __launch_bounds__(FFT_T) fft_x_adjoint_kernel(FftGeom g, const f
     const int iz = min(col0 + col, g.N[2] / 2);
     const float kty = (float)g.ktab[3 * g.tabn + iy], ktz = (float)g.ktab[6 * g.tabn + iz];
     load_tw(tw, g.twx, NX);
-    for (int i = threadIdx.x; i < NX; i += FFT_T) ktx[i] = (float)g.ktab[i];
+    for (int i = threadIdx.x; i < NX; i += FFT_T) {
+        ktx[i] = (float)g.ktab[i];
+        k2x[i] = g.ktab[g.tabn + i];
+        decx[i] = g.ktab[2 * g.tabn + i];
+    }
     // kt_y and kt_z do not depend on x: kt_y Pi_y + kt_z Pi_z is formed BEFORE the transform along x, so two forward
     // transforms (Pi_x and that sum) instead of three
     tile_load<NX, CS>(accum, Pi + g.cstride + off, stride, ncol);
@@ -333,11 +359,12 @@ __global__ void __launch_bounds__(FFT_T) fft_x_adjoint_kernel(FftGeom g, const f
     __syncthreads();
     AxisFFT<NX, NX, false, B, CS>::run(work, ncol, tw);
     if (col < ncol) {
+        const GreenCol gc = green_col(g, iy, iz);
 #pragma unroll 4
         for (int pos = threadIdx.x >> CS; pos < NX; pos += FFT_T >> CS) {
             const float c = ktx[pos];
             const float2 v = work[(pos << CS) + col], a = accum[(pos << CS) + col];
-            const float G = mode_green(g, pos, iy, iz);
+            const float G = mode_green(gc, k2x[pos], decx[pos]);
             // times -i G: (re, im) -> (G im, -G re)
             accum[(pos << CS) + col] = make_float2(G * (c * v.y + a.y), -G * (c * v.x + a.x));
         }
@@ -653,7 +680,7 @@ static int fft_x_fused(pm_ctx *c, const float *in, float *out, double nbar, bool
     fg.c0 = 1.5 * c->prm.omega_m / (nbar * (double)g.ng);
     const int cs = g.N[0] <= 256 ? 4 : (g.N[0] <= 512 ? 3 : 2), B = 1 << cs;  // two tiles of Nx x B: keep 3 CTAs per SM
     dim3 grid((unsigned)((fg.zsc + B - 1) / B), (unsigned)g.N[1]);
-    size_t smem = sizeof(float2) * ((size_t)g.N[0] + 2 * (size_t)g.N[0] * B) + sizeof(float) * (size_t)g.N[0];
+    size_t smem = sizeof(float2) * ((size_t)g.N[0] + 2 * (size_t)g.N[0] * B) + (2 * sizeof(double) + sizeof(float)) * (size_t)g.N[0];
     Timer t(c, adjoint ? TC_KSPACE_ADJ : TC_KSPACE_FORCE, 32.0 * (double)g.nk);
 #define X_CASE(NN, CS_)                                                                                                                   \
     if (adjoint) PM_FFT_LAUNCH(c, "fft_x_adjoint_kernel", (fft_x_adjoint_kernel<NN, CS_>), grid, smem, fg, (const float2 *)in, (float2 *)out); \
