@@ -408,7 +408,7 @@ __global__ void __launch_bounds__(FFT_T) fft_z_r2c_kernel(FftGeom g, float *data
         const int r = threadIdx.x & (ZROWS - 1);
         if (r < nr) {
 #pragma unroll 4
-            for (int n = threadIdx.x >> ZRS; n < M; n += FFT_T >> ZRS) tile[n * ZP + r] = *reinterpret_cast<const float2 *>(stage + r * zs + 2 * n);
+            for (int n = threadIdx.x >> ZRS; n < M; n += FFT_T >> ZRS) tile[n * ZP + r] = *reinterpret_cast<const float2 *>(stage + r * (2 * M + 4) + 2 * n);
         }
     }
     __syncthreads();
@@ -430,7 +430,7 @@ __global__ void __launch_bounds__(FFT_T) fft_z_r2c_kernel(FftGeom g, float *data
     __syncthreads();
     float2 *crow = reinterpret_cast<float2 *>(rows);
     for (int r = threadIdx.x / 64; r < nr; r += FFT_T / 64)
-        for (int k = threadIdx.x & 63; k < g.zsc; k += 64) crow[(size_t)r * g.zsc + k] = k <= M ? outb[k * ZP + r] : make_float2(0.f, 0.f);
+        for (int k = threadIdx.x & 63; k < M + 2; k += 64) crow[r * (M + 2) + k] = k <= M ? outb[k * ZP + r] : make_float2(0.f, 0.f);  // zsc = M + 2
 }
 
 // ---- z pass, half-complex -> real (unnormalised: Nz times the inverse), in place ------------------------------
@@ -464,7 +464,7 @@ __global__ void __launch_bounds__(FFT_T) fft_z_c2r_kernel(FftGeom g, float *data
         if (r < nr) {
 #pragma unroll 4
             for (int k = threadIdx.x >> ZRS; k < M; k += FFT_T >> ZRS) {
-                const float2 a = inb[r * g.zsc + k], b = inb[r * g.zsc + M - k];
+                const float2 a = inb[r * (M + 2) + k], b = inb[r * (M + 2) + M - k];
                 const float2 E = make_float2(a.x + b.x, a.y - b.y);
                 const float2 O = cmulc(make_float2(a.x - b.x, a.y + b.y), twr[k]);
                 tile[posz[k] * ZP + r] = make_float2(E.x - O.y, E.y + O.x);  // E + i O
@@ -477,7 +477,7 @@ __global__ void __launch_bounds__(FFT_T) fft_z_c2r_kernel(FftGeom g, float *data
         constexpr int RPP = FFT_T / M > 0 ? FFT_T / M : 1;
         const int n = threadIdx.x % M, r0 = threadIdx.x / M;
 #pragma unroll 4
-        for (int r = r0; r < nr; r += RPP) *reinterpret_cast<float2 *>(rows + (size_t)r * zs + 2 * n) = tile[n * ZP + r];
+        for (int r = r0; r < nr; r += RPP) *reinterpret_cast<float2 *>(rows + r * (2 * M + 4) + 2 * n) = tile[n * ZP + r];  // zs = 2 M + 4
     } else {
         for (int r = 0; r < nr; r++)
             for (int n = threadIdx.x; n < M; n += FFT_T) *reinterpret_cast<float2 *>(rows + (size_t)r * zs + 2 * n) = tile[n * ZP + r];
