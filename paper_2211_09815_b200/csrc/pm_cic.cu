@@ -853,14 +853,23 @@ __global__ void __launch_bounds__(GT) gather_kernel(CicGeom g, const uint4 *__re
         uint4 q_nx = make_uint4(0, 0, 0, 0);
         const bool has_nx = nxt.tile >= 0 && nxt.beg + tid < nxt.end;
         if (has_nx) q_nx = rec[nxt.beg + tid];
+        // a second round of the current tile (more than GT particles): its record is requested now, its per-particle
+        // inputs right after the barrier, so that neither round trip is exposed between the rounds
+        const int cnt = (g.dbg & 1) ? 0 : cur.end - cur.beg;
+        uint4 q2 = make_uint4(0, 0, 0, 0);
+        if (tid + GT < cnt) q2 = rec[cur.beg + tid + GT];
         cp_async_wait<GST - 1>();  // this thread's copies of the current tile have landed ...
         __syncthreads();     // ... and everybody else's
+        PIn pin2;
+        if (tid + GT < cnt) pin2.load(q2.w, cot, ka);
 
         const int t0[3] = {cur.t0[0], cur.t0[1], cur.t0[2]};
         const float *halo = halo_of(n % GST);
-        const int cnt = (g.dbg & 1) ? 0 : cur.end - cur.beg;
         for (int i = tid; i < cnt; i += GT) {
-            if (i != tid) {
+            if (i == tid + GT) {
+                q = q2;
+                pin = pin2;
+            } else if (i != tid) {
                 q = rec[cur.beg + i];
                 pin.load(q.w, cot, ka);
             }
