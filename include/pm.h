@@ -77,6 +77,11 @@ int pm_host_growth(double omega_m, double a, double out[4]);
 /*   the three factors of a forward KDK step a_prev -> a_next (eq. 16; eq. 15), with
  *   a_half = (a_prev + a_next)/2: out = {K(a_prev; a_prev, a_half), D(a_half; a_prev, a_next), K(a_next; a_half, a_next)} */
 int pm_host_step_factors(double omega_m, double a_prev, double a_next, double out[3]);
+/*   memory order of the library's own FFT passes along an axis of n points (n a power of two, 8 <= n <= 1024):
+ *   out[p] = frequency index (0 .. n-1, e^{-2 pi i k g / n} convention) that memory position p holds after the
+ *   forward decimation-in-frequency stages (radix 16, ..., then the remainder).  Pure host; the k-space tables are
+ *   built from it and nothing in k-space crosses this ABI (R26). */
+int pm_host_fft_order(int32_t n, int32_t *out);
 /*   the factors stored in ctx for forward step i in 1..n; the adjoint step uses their exact negatives (L389) */
 int pm_step_factors(const pm_ctx *ctx, int i, double out[3]);
 

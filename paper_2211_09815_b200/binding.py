@@ -49,6 +49,7 @@ _SIGS = {
     "pm_host_growth": (_int, [_dbl, _dbl, C.POINTER(_dbl)]),
     "pm_host_step_factors": (_int, [_dbl, _dbl, _dbl, C.POINTER(_dbl)]),
     "pm_step_factors": (_int, [_vp, _int, C.POINTER(_dbl)]),
+    "pm_host_fft_order": (_int, [C.c_int32, C.POINTER(C.c_int32)]),
     "pm_scatter": (_int, [_vp, _i64, _vp, _vp, _int, _vp]),
     "pm_gather": (_int, [_vp, _i64, _vp, _vp, _int, _vp]),
     "pm_gather_grad": (_int, [_vp, _i64, _vp, _vp, _int, _vp, _vp]),
@@ -112,6 +113,15 @@ def host_step_factors(omega_m, a_prev, a_next):
     rc = _lib.pm_host_step_factors(float(omega_m), float(a_prev), float(a_next), out)
     if rc != PM_OK:
         raise PMError(rc, "pm_host_step_factors")
+    return list(out)
+
+
+def host_fft_order(n):
+    """Frequency index held at each memory position after the own FFT's forward stages along an n-point axis (pure host)."""
+    out = (C.c_int32 * int(n))()
+    rc = _lib.pm_host_fft_order(int(n), out)
+    if rc != PM_OK:
+        raise PMError(rc, "pm_host_fft_order")
     return list(out)
 
 

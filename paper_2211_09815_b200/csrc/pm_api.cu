@@ -378,6 +378,8 @@ int pm_host_step_factors(double omega_m, double a0, double a1, double out[3])
     return PM_OK;
 }
 
+int pm_host_fft_order(int32_t n, int32_t *out) { return fft_own_order_host((int)n, (int *)out); }
+
 int pm_step_factors(const pm_ctx *c, int i, double out[3])
 {
     if (!c || !out || i < 1 || i > c->prm.n_steps) return PM_EINVAL;

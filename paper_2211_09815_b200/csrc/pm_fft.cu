@@ -548,6 +548,15 @@ void fft_own_axis_order(const pm_ctx *c, int axis, std::vector<int> &freq)
     }
 }
 
+// host-only view of the same table for the ABI (include/pm.h: pm_host_fft_order)
+int fft_own_order_host(int n, int *out)
+{
+    if (!out || !is_pow2(n) || n < 8 || n > 1024) return PM_EINVAL;
+    AxisPlan p = make_axis_plan(n);
+    for (int i = 0; i < n; i++) out[i] = freq_of_pos(p, i);
+    return PM_OK;
+}
+
 static FftGeom *geom_of(pm_ctx *c) { return reinterpret_cast<FftGeom *>(c->fft_geom); }
 
 int fft_own_init(pm_ctx *c)

@@ -183,6 +183,7 @@ int kspace_adjoint(pm_ctx *c, const float2 *Pi_k /*3 meshes*/, float2 *psi_k, do
 // ---- own FFT with fused k-space operators (pm_fft.cu) ------------------------------------------------
 bool fft_own_supported(const Geometry &g);
 size_t fft_own_table_bytes(const Geometry &g);
+int fft_own_order_host(int n, int *out);
 int fft_own_init(pm_ctx *c);                                  // needs c->ktab, c->fft_tab carved
 void fft_own_axis_order(const pm_ctx *c, int axis, std::vector<int> &freq);  // frequency index stored at each memory position
 int fft_own_force(pm_ctx *c, float *rho, float *f3, double nbar, int part = 0);     // part: see pm_fft.cu

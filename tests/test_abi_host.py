@@ -89,3 +89,30 @@ def test_host_growth_matches_oracle_ode(binding, orc, om):
         ah = 0.5 * (a0 + a1)
         ref = [orc.kick_factor(om, a0, a0, ah), orc.drift_factor(om, ah, a0, a1), orc.kick_factor(om, a1, ah, a1)]
         np.testing.assert_allclose(binding.host_step_factors(om, a0, a1), ref, rtol=2e-8)
+
+
+def test_own_fft_memory_order_is_the_dif_digit_reversal(binding):
+    """pm_host_fft_order against an independent numpy run of the same in-place decimation-in-frequency schedule
+    (radix min(16, L) per stage, csrc/pm_fft.cu): position p of the staged result must hold numpy.fft.fft's bin out[p]."""
+    rng = np.random.default_rng(3)
+    for n in (8, 16, 32, 64, 128, 256, 512, 1024):
+        order = np.asarray(binding.host_fft_order(n))
+        assert sorted(order.tolist()) == list(range(n))                  # a permutation
+        x = rng.standard_normal(n) + 1j * rng.standard_normal(n)
+        y = x.copy()
+        L = n
+        while L > 1:
+            R = min(16, L)
+            Lr = L // R
+            for blk in range(n // L):
+                for j in range(Lr):
+                    idx = blk * L + j + Lr * np.arange(R)
+                    a = y[idx]
+                    q = np.arange(R)
+                    # R-point DFT over m, then the stage twiddle w_L^(j q), stored at blk L + j + q L/R
+                    y[idx] = (np.exp(-2j * np.pi * np.outer(q, np.arange(R)) / R) @ a) * np.exp(-2j * np.pi * j * q / L)
+            L = Lr
+        ref = np.fft.fft(x)
+        assert np.allclose(y, ref[order], rtol=1e-10, atol=1e-10), n
+    with pytest.raises(binding.PMError):
+        binding.host_fft_order(48)
