@@ -23,6 +23,16 @@ int fail(pm_ctx *c, int code, const char *what, const char *detail)
     return code;
 }
 
+bool pdl_enabled()
+{
+    static int v = -1;
+    if (v < 0) {
+        const char *e = getenv("PM_PDL");
+        v = (e && atoi(e) == 0) ? 0 : 1;
+    }
+    return v == 1;
+}
+
 Timer::Timer(pm_ctx *ctx, int cls, double bytes) : c(ctx), idx(-1)
 {
     if (cls == TC_FFT_R2C || cls == TC_FFT_C2R) c->n_fft++; else c->n_own++;

@@ -67,6 +67,7 @@ template <bool FROM_STATE>
 __global__ void __launch_bounds__(256) bin_count_kernel(PosGeom g, long long np, const float *__restrict__ x,
                                                         const long long *__restrict__ xs, int *__restrict__ hist)
 {
+    pdl_enter();
     long long stride = (long long)gridDim.x * blockDim.x;
     for (long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x; j < np; j += stride) {
         unsigned int X[3];
@@ -80,6 +81,7 @@ __global__ void __launch_bounds__(256) bin_reorder_kernel(PosGeom g, long long n
                                                           const long long *__restrict__ xs, int *__restrict__ cursor,
                                                           uint4 *__restrict__ rec)
 {
+    pdl_enter();
     long long stride = (long long)gridDim.x * blockDim.x;
     long long n_round = (np + 31) / 32 * 32;
     for (long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x; j < n_round; j += stride) {
@@ -136,6 +138,7 @@ __global__ void __launch_bounds__(SCAN_T) scan_kernel(int *__restrict__ hist, in
 {
     __shared__ int tot;
     __shared__ int base_s;
+    pdl_enter();
     const int base = blockIdx.x * SCAN_CH + threadIdx.x * SCAN_PER;
     int v[SCAN_PER], sum = 0;
     if (base + SCAN_PER <= n) {
@@ -196,9 +199,9 @@ int bin_count(pm_ctx *c, long long np, const float *x)
     PosGeom b = make_pos_geom(c->g);
     Timer t(c, TC_BIN_COUNT, (x ? 12.0 : 24.0) * np);
     if (x)
-        bin_count_kernel<false><<<bin_blocks(np), 256, 0, c->stream>>>(b, np, x, nullptr, c->hist);
+        PM_CUDA(c, launch_pdl(bin_count_kernel<false>, dim3(bin_blocks(np)), dim3(256), 0, c->stream, b, np, x, nullptr, c->hist));
     else
-        bin_count_kernel<true><<<bin_blocks(np), 256, 0, c->stream>>>(b, np, nullptr, c->x, c->hist);
+        PM_CUDA(c, launch_pdl(bin_count_kernel<true>, dim3(bin_blocks(np)), dim3(256), 0, c->stream, b, np, nullptr, c->x, c->hist));
     PM_LAUNCH_CHECK(c, "bin_count_kernel");
     t.stop();
     return PM_OK;
@@ -215,16 +218,16 @@ int bin_sort(pm_ctx *c, long long np, const float *x)
         int nb = (n + SCAN_CH - 1) / SCAN_CH;
         c->scan_epoch++;
         if (c->scan_epoch == 0) c->scan_epoch = 1;  // 0 is the tag of the zero-initialised buffer
-        scan_kernel<<<nb, SCAN_T, 0, c->stream>>>(c->hist, n, c->offsets, c->cursor, c->scan_agg, c->scan_epoch);
+        PM_CUDA(c, launch_pdl(scan_kernel, dim3(nb), dim3(SCAN_T), 0, c->stream, c->hist, n, c->offsets, c->cursor, c->scan_agg, c->scan_epoch));
         PM_LAUNCH_CHECK(c, "scan kernels");
         t.stop();
     }
     {
         Timer t(c, TC_BIN_REORDER, (x ? 28.0 : 40.0) * np);
         if (x)
-            bin_reorder_kernel<false><<<bin_blocks(np), 256, 0, c->stream>>>(b, np, x, nullptr, c->cursor, c->rec);
+            PM_CUDA(c, launch_pdl(bin_reorder_kernel<false>, dim3(bin_blocks(np)), dim3(256), 0, c->stream, b, np, x, nullptr, c->cursor, c->rec));
         else
-            bin_reorder_kernel<true><<<bin_blocks(np), 256, 0, c->stream>>>(b, np, nullptr, c->x, c->cursor, c->rec);
+            PM_CUDA(c, launch_pdl(bin_reorder_kernel<true>, dim3(bin_blocks(np)), dim3(256), 0, c->stream, b, np, nullptr, c->x, c->cursor, c->rec));
         PM_LAUNCH_CHECK(c, "bin_reorder_kernel");
         t.stop();
     }

@@ -370,6 +370,7 @@ __global__ void __launch_bounds__(NTHREADS) scatter_kernel(const __grid_constant
         mbar_fence_init();
     }
     __syncthreads();
+    pdl_enter();
 
     if (warp == NCW) {
         // ---------------- producer warp ----------------
@@ -796,6 +797,7 @@ __global__ void __launch_bounds__(GT) gather_kernel(CicGeom g, const uint4 *__re
     // thread 0 draws tiles from the global counter and publishes them two iterations ahead.  The chain
     // atomic -> offsets -> slot is software-pipelined: every iteration consumes what the previous one requested
     // (the tile index of the atomic, the offsets of the tile drawn before), so no round trip is exposed.
+    pdl_enter();
     int d_tile = 0, d_beg = 0, d_end = 0, d_atom = 0;  // thread 0 only: tile with offsets in flight; atomic in flight
     auto draw_request = [&]() {
         d_tile = d_atom;
@@ -1000,7 +1002,7 @@ static cudaError_t allow_smem(K kernel, size_t bytes)
             PM_CUDA(ctx, allow_smem(kernel, smem));                                          \
             attr_done_ = true;                                                               \
         }                                                                                    \
-        kernel<<<persistent_grid(ctx, smem, threads), threads, smem, (ctx)->stream>>>(__VA_ARGS__); \
+        PM_CUDA(ctx, launch_pdl(kernel, dim3(persistent_grid(ctx, smem, threads)), dim3(threads), smem, (ctx)->stream, __VA_ARGS__)); \
         PM_LAUNCH_CHECK(ctx, name);                                                          \
     } while (0)
 

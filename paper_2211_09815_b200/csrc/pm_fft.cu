@@ -207,6 +207,7 @@ template <int NY, int CS, bool INV>
 __global__ void __launch_bounds__(FFT_T) fft_y_kernel(FftGeom g, float2 *data)
 {
     extern __shared__ __align__(16) unsigned char fsm[];
+    pdl_enter();
     float2 *tile = reinterpret_cast<float2 *>(fsm);
     float2 *tw = tile + (NY << CS);
     constexpr int B = 1 << CS;
@@ -250,6 +251,7 @@ template <int NX, int CS>
 __global__ void __launch_bounds__(FFT_T) fft_x_force_kernel(FftGeom g, const float2 *rho, float2 *f)
 {
     extern __shared__ __align__(16) unsigned char fsm[];
+    pdl_enter();
     constexpr int B = 1 << CS;
     float2 *spec = reinterpret_cast<float2 *>(fsm);
     float2 *work = spec + (NX << CS);
@@ -320,6 +322,7 @@ template <int NX, int CS>
 __global__ void __launch_bounds__(FFT_T) fft_x_adjoint_kernel(FftGeom g, const float2 *Pi, float2 *psi)
 {
     extern __shared__ __align__(16) unsigned char fsm[];
+    pdl_enter();
     constexpr int B = 1 << CS;
     float2 *accum = reinterpret_cast<float2 *>(fsm);
     float2 *work = accum + (NX << CS);
@@ -383,6 +386,7 @@ __global__ void __launch_bounds__(FFT_T) fft_z_r2c_kernel(FftGeom g, float *data
 {
     constexpr int ZROWS = 1 << ZRS, ZP = ZROWS + 1;  // z-rows per CTA; tile pitch
     extern __shared__ __align__(16) unsigned char fsm[];
+    pdl_enter();
     float2 *tile = reinterpret_cast<float2 *>(fsm);
     float2 *outb = tile + M * ZP;
     float2 *tw = outb + max((M + 1) * ZP, ZROWS * g.zsc);
@@ -441,6 +445,7 @@ __global__ void __launch_bounds__(FFT_T) fft_z_c2r_kernel(FftGeom g, float *data
 {
     constexpr int ZROWS = 1 << ZRS, ZP = ZROWS + 1;  // z-rows per CTA; tile pitch
     extern __shared__ __align__(16) unsigned char fsm[];
+    pdl_enter();
     float2 *tile = reinterpret_cast<float2 *>(fsm);
     float2 *inb = tile + M * ZP;
     float2 *tw = inb + max((M + 1) * ZP, ZROWS * g.zsc);
@@ -606,7 +611,7 @@ int fft_own_init(pm_ctx *c)
             PM_CUDA(ctx, cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(smem))); \
             attr_ = (smem);                                                                \
         }                                                                                  \
-        kernel<<<grid, FFT_T, smem, (ctx)->stream>>>(__VA_ARGS__);                         \
+        PM_CUDA(ctx, launch_pdl(kernel, dim3(grid), dim3(FFT_T), smem, (ctx)->stream, __VA_ARGS__)); \
         PM_LAUNCH_CHECK(ctx, name);                                                        \
     } while (0)
 

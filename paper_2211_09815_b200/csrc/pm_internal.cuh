@@ -6,6 +6,7 @@
 #include <cufft.h>
 #include <stdint.h>
 #include <string>
+#include <utility>
 #include <vector>
 
 #include "pm.h"
@@ -139,6 +140,34 @@ int fail(pm_ctx *c, int code, const char *what, const char *detail);
         int rc_ = (expr);            \
         if (rc_ != PM_OK) return rc_; \
     } while (0)
+
+// ---- programmatic dependent launch (PDL) ------------------------------------------------------------
+// Kernels launched through launch_pdl may be scheduled while the previous kernel of the stream is still draining;
+// each of them calls pdl_enter() before it touches anything a predecessor wrote (it also lets ITS successor in).
+// What overlaps is the launch latency, the CTA ramp-up and the prologue with the predecessor's tail.  PM_PDL=0 disables.
+#ifdef __CUDACC__
+__device__ __forceinline__ void pdl_enter()
+{
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+}
+#endif
+bool pdl_enabled();
+template <class... KArgs, class... Args>
+inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args &&...args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = pdl_enabled() ? 1 : 0;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, std::forward<Args>(args)...);
+}
 
 // RAII-ish bracket: t = Timer(ctx, cls, bytes); launch...; t.stop()
 struct Timer {
