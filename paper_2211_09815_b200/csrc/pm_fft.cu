@@ -207,14 +207,15 @@ template <int NY, int CS, bool INV>
 __global__ void __launch_bounds__(FFT_T) fft_y_kernel(FftGeom g, float2 *data)
 {
     extern __shared__ __align__(16) unsigned char fsm[];
-    pdl_enter();
+    pdl_trigger();  // the constant tables are loaded before pdl_wait(), the data after it
     float2 *tile = reinterpret_cast<float2 *>(fsm);
     float2 *tw = tile + (NY << CS);
     constexpr int B = 1 << CS;
     const int col0 = blockIdx.x * B, ncol = min(B, g.zsc - col0);
     float2 *base = data + (size_t)blockIdx.z * g.cstride + (size_t)blockIdx.y * NY * g.zsc + col0;
-    tile_load<NY, CS>(tile, base, g.zsc, ncol);
     load_tw(tw, g.twy, NY);
+    pdl_wait();
+    tile_load<NY, CS>(tile, base, g.zsc, ncol);
     fft_cp_async_wait_all();
     __syncthreads();
     AxisFFT<NY, NY, INV, B, CS>::run(tile, ncol, tw);
@@ -251,7 +252,7 @@ template <int NX, int CS>
 __global__ void __launch_bounds__(FFT_T) fft_x_force_kernel(FftGeom g, const float2 *rho, float2 *f)
 {
     extern __shared__ __align__(16) unsigned char fsm[];
-    pdl_enter();
+    pdl_trigger();  // the constant tables are loaded before pdl_wait(), the data after it
     constexpr int B = 1 << CS;
     float2 *spec = reinterpret_cast<float2 *>(fsm);
     float2 *work = spec + (NX << CS);
@@ -262,13 +263,14 @@ __global__ void __launch_bounds__(FFT_T) fft_x_force_kernel(FftGeom g, const flo
     const int iy = blockIdx.y;
     const long long stride = (long long)g.N[1] * g.zsc;
     const size_t off = (size_t)iy * g.zsc + col0;
-    tile_load<NX, CS>(spec, rho + off, stride, ncol);
     load_tw(tw, g.twx, NX);
     for (int i = threadIdx.x; i < NX; i += FFT_T) {
         ktx[i] = (float)g.ktab[i];
         k2x[i] = g.ktab[g.tabn + i];
         decx[i] = g.ktab[2 * g.tabn + i];
     }
+    pdl_wait();
+    tile_load<NX, CS>(spec, rho + off, stride, ncol);
     fft_cp_async_wait_all();
     __syncthreads();
     AxisFFT<NX, NX, false, B, CS>::run(spec, ncol, tw);
@@ -322,7 +324,7 @@ template <int NX, int CS>
 __global__ void __launch_bounds__(FFT_T) fft_x_adjoint_kernel(FftGeom g, const float2 *Pi, float2 *psi)
 {
     extern __shared__ __align__(16) unsigned char fsm[];
-    pdl_enter();
+    pdl_trigger();  // the constant tables are loaded before pdl_wait(), the data after it
     constexpr int B = 1 << CS;
     float2 *accum = reinterpret_cast<float2 *>(fsm);
     float2 *work = accum + (NX << CS);
@@ -342,6 +344,7 @@ __global__ void __launch_bounds__(FFT_T) fft_x_adjoint_kernel(FftGeom g, const f
         k2x[i] = g.ktab[g.tabn + i];
         decx[i] = g.ktab[2 * g.tabn + i];
     }
+    pdl_wait();
     // kt_y and kt_z do not depend on x: kt_y Pi_y + kt_z Pi_z is formed BEFORE the transform along x, so two forward
     // transforms (Pi_x and that sum) instead of three
     tile_load<NX, CS>(accum, Pi + g.cstride + off, stride, ncol);
@@ -386,7 +389,7 @@ __global__ void __launch_bounds__(FFT_T) fft_z_r2c_kernel(FftGeom g, float *data
 {
     constexpr int ZROWS = 1 << ZRS, ZP = ZROWS + 1;  // z-rows per CTA; tile pitch
     extern __shared__ __align__(16) unsigned char fsm[];
-    pdl_enter();
+    pdl_trigger();  // the constant tables are loaded before pdl_wait(), the data after it
     float2 *tile = reinterpret_cast<float2 *>(fsm);
     float2 *outb = tile + M * ZP;
     float2 *tw = outb + max((M + 1) * ZP, ZROWS * g.zsc);
@@ -399,13 +402,14 @@ __global__ void __launch_bounds__(FFT_T) fft_z_r2c_kernel(FftGeom g, float *data
     // the nr rows are contiguous in memory: 16-byte async copies into a row-major staging area (which shares its
     // shared memory with outb), then the transposing fill of the tile
     float *stage = reinterpret_cast<float *>(outb);
+    load_tw(tw, g.twz, M);
+    load_tw(twr, g.twzr, M + 1);
+    for (int i = threadIdx.x; i < M; i += FFT_T) posz[i] = g.posz[i];
+    pdl_wait();
     {
         const int nchunk = nr * (zs / 4);
         for (int i = threadIdx.x; i < nchunk; i += FFT_T) fft_cp_async16(stage + 4 * i, rows + 4 * (size_t)i);
     }
-    load_tw(tw, g.twz, M);
-    load_tw(twr, g.twzr, M + 1);
-    for (int i = threadIdx.x; i < M; i += FFT_T) posz[i] = g.posz[i];
     fft_cp_async_wait_all();
     __syncthreads();
     {
@@ -445,7 +449,7 @@ __global__ void __launch_bounds__(FFT_T) fft_z_c2r_kernel(FftGeom g, float *data
 {
     constexpr int ZROWS = 1 << ZRS, ZP = ZROWS + 1;  // z-rows per CTA; tile pitch
     extern __shared__ __align__(16) unsigned char fsm[];
-    pdl_enter();
+    pdl_trigger();  // the constant tables are loaded before pdl_wait(), the data after it
     float2 *tile = reinterpret_cast<float2 *>(fsm);
     float2 *inb = tile + M * ZP;
     float2 *tw = inb + max((M + 1) * ZP, ZROWS * g.zsc);
@@ -455,13 +459,14 @@ __global__ void __launch_bounds__(FFT_T) fft_z_c2r_kernel(FftGeom g, float *data
     const long long row0 = (long long)blockIdx.x * ZROWS;
     const int nr = (int)min((long long)ZROWS, nrows - row0);
     float *rows = data + (size_t)row0 * zs;
+    load_tw(tw, g.twz, M);
+    load_tw(twr, g.twzr, M + 1);
+    for (int i = threadIdx.x; i < M; i += FFT_T) posz[i] = g.posz[i];
+    pdl_wait();
     {   // the nr rows are contiguous in memory: 16-byte async copies, row-major [row][zsc]
         const int nchunk = nr * (zs / 4);
         for (int i = threadIdx.x; i < nchunk; i += FFT_T) fft_cp_async16(reinterpret_cast<float *>(inb) + 4 * i, rows + 4 * (size_t)i);
     }
-    load_tw(tw, g.twz, M);
-    load_tw(twr, g.twzr, M + 1);
-    for (int i = threadIdx.x; i < M; i += FFT_T) posz[i] = g.posz[i];
     fft_cp_async_wait_all();
     __syncthreads();
     {

@@ -146,10 +146,12 @@ int fail(pm_ctx *c, int code, const char *what, const char *detail);
 // each of them calls pdl_enter() before it touches anything a predecessor wrote (it also lets ITS successor in).
 // What overlaps is the launch latency, the CTA ramp-up and the prologue with the predecessor's tail.  PM_PDL=0 disables.
 #ifdef __CUDACC__
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ void pdl_enter()
 {
-    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-    asm volatile("griddepcontrol.wait;" ::: "memory");
+    pdl_trigger();
+    pdl_wait();
 }
 #endif
 bool pdl_enabled();
