@@ -47,6 +47,7 @@ struct CicGeom {
     double mean;   // unit-mass scatter only: constant subtracted from every mesh point IN INTEGER, before the
                    // int -> fp32 conversion (0 = plain density; nbar on the force path, whose k = 0 mode is zeroed
                    // anyway, so that fp32 rounding is relative to the fluctuation rho - nbar, not to rho)
+    long long *dbgbuf;  // debug timeline (PM_DEBUG_CIC & 8): clock64 stamps of CTA 0
     int *sched;    // [0] tile counter, [1] finished CTAs; both zero between launches (the last CTA resets them)
 };
 
@@ -188,6 +189,7 @@ static CicGeom make_cic_geom(pm_ctx *c, const float *mesh, int C, int zs, long l
     { const char *e = getenv("PM_DEBUG_TMA_HALO"); r.tma_halo = e ? atoi(e) : 0; }
     { const char *e = getenv("PM_DEBUG_CIC"); r.dbg = e ? atoi(e) : 0; }
     r.sched = c->sched;
+    r.dbgbuf = reinterpret_cast<long long *>(c->scal);
     memset(map, 0, sizeof(*map));
     long long off = mesh - c->mesh[0];
     bool internal = zs == g.zs && ms == g.mesh_stride && mesh >= c->mesh[0] && off % g.mesh_stride == 0 &&
@@ -671,7 +673,7 @@ __global__ void __launch_bounds__(NTHREADS) scatter_kernel(const __grid_constant
 // two-stage cp.async pipeline: every thread first starts the copies of the NEXT tile's halo, then interpolates
 // for the particles of the current one.
 enum GatherMode { G_VALUE = 0, G_GRAD = 1, G_FUSED = 2 };
-constexpr int GT = 256;                                    // threads of a gather CTA
+constexpr int GT = 320;                                    // threads of a gather CTA
 constexpr int GCH = HZP / 4;                               // 16-byte pieces per halo row (9)
 constexpr int GRG = GT / GCH;                              // halo rows covered per pass of the CTA (28)
 
@@ -798,33 +800,43 @@ __global__ void __launch_bounds__(GT) gather_kernel(CicGeom g, const uint4 *__re
     // atomic -> offsets -> slot is software-pipelined: every iteration consumes what the previous one requested
     // (the tile index of the atomic, the offsets of the tile drawn before), so no round trip is exposed.
     pdl_enter();
-    int d_tile = 0, d_beg = 0, d_end = 0, d_atom = 0;  // thread 0 only: tile with offsets in flight; atomic in flight
-    auto draw_request = [&]() {
-        d_tile = d_atom;
-        if (d_tile < g.ntiles) {
-            d_beg = offsets[d_tile * NCLS];
-            d_end = offsets[d_tile * NCLS + NCLS];
+    // The tiles are drawn by the LAST thread: its warp has particles only in tiles with more than GT - 32 of them, so the
+    // round trips of the draw rarely sit on the critical path to the barrier (warp 0 always has the most particles).
+    constexpr int DRAWER = GT - 1;
+    // The pipeline registers come in two sets used by alternate iterations (the loop body is instantiated twice): a
+    // freshly requested value is then never copied at the loop's back edge, which would wait for its round trip.
+    struct DrawSet { int tile, beg, end; };
+    DrawSet S0 = {0, 0, 0}, S1 = {0, 0, 0};  // drawing thread only: tile whose offsets are in flight
+    int a0 = 0, a1 = 0;                      // drawing thread only: tile index of the atomic in flight
+    auto draw_request = [&](DrawSet &fill, const int &a_use, int &a_new) {
+        fill.tile = a_use;
+        if (fill.tile < g.ntiles) {
+            fill.beg = offsets[fill.tile * NCLS];
+            fill.end = offsets[fill.tile * NCLS + NCLS];
         }
-        d_atom = atomicAdd(&g.sched[0], 1);
+        a_new = atomicAdd(&g.sched[0], 1);
     };
-    auto draw_publish = [&](GatherSlot &dst) {
-        dst.tile = d_tile < g.ntiles ? d_tile : -1;
-        dst.beg = d_beg;
-        dst.end = d_end;
-        if (d_tile < g.ntiles) {
+    auto draw_publish = [&](GatherSlot &dst, const DrawSet &d) {
+        dst.tile = d.tile < g.ntiles ? d.tile : -1;
+        dst.beg = d.beg;
+        dst.end = d.end;
+        if (d.tile < g.ntiles) {
             int tt[3], tt0[3], text[3];
-            tile_coords(g, d_tile, tt, tt0, text);
+            tile_coords(g, d.tile, tt, tt0, text);
 #pragma unroll
-            for (int d = 0; d < 3; d++) { dst.t0[d] = tt0[d]; dst.ext[d] = text[d]; }
+            for (int k = 0; k < 3; k++) { dst.t0[k] = tt0[k]; dst.ext[k] = text[k]; }
         }
     };
-    if (tid == 0) {
-        d_atom = atomicAdd(&g.sched[0], 1);
-        draw_request();
+    if (tid == DRAWER) {
+        // prologue (latencies exposed once): after it S0 holds the tile to publish at iteration 0 and a0 the next index
+        int a = atomicAdd(&g.sched[0], 1), b = 0;
+        draw_request(S0, a, b);
         for (int k = 0; k < PUB; k++) {
-            draw_publish(slot[k]);
-            draw_request();
+            draw_publish(slot[k], S0);
+            a = b;
+            draw_request(S0, a, b);
         }
+        a0 = b;
     }
     __syncthreads();
     for (int k = 0; k < GST - 1; k++) {
@@ -841,10 +853,12 @@ __global__ void __launch_bounds__(GT) gather_kernel(CicGeom g, const uint4 *__re
 
     const float fr = 1.f / (float)(1u << g.fbits);
     const unsigned fmask = (1u << g.fbits) - 1u;
-    for (int n = 0;; n++) {
+    auto body = [&](const int n, DrawSet &Spub, DrawSet &Sfill, int &a_use, int &a_new) -> bool {
         const GatherSlot cur = slot[n & 7];
-        if (cur.tile < 0) break;
-        const GatherSlot nxt = slot[(n + 1) & 7];
+        if (cur.tile < 0) return false;
+#define PM_STAMP(k) do { if ((g.dbg & 8) && blockIdx.x == 0 && n < 40 && (tid == 0 || tid == GT - 1)) g.dbgbuf[((tid ? 1 : 0) * 40 + n) * 12 + (k)] = clock64(); } while (0)
+        PM_STAMP(0);
+        if ((g.dbg & 8) && blockIdx.x == 0 && n < 40 && tid == 0) g.dbgbuf[n * 12 + 11] = cur.end - cur.beg;
         // the halo of the tile GST - 1 iterations ahead starts to fly now (its stage was released by the barrier that
         // ended iteration n - 1)
         {
@@ -852,6 +866,8 @@ __global__ void __launch_bounds__(GT) gather_kernel(CicGeom g, const uint4 *__re
             if (far.tile >= 0 && far.beg < far.end && !(g.dbg & 2)) halo_issue<C>(g, mesh, far, halo_of((n + GST - 1) % GST));
         }
         cp_async_commit();
+        PM_STAMP(1);
+        const GatherSlot nxt = slot[(n + 1) & 7];
         uint4 q_nx = make_uint4(0, 0, 0, 0);
         const bool has_nx = nxt.tile >= 0 && nxt.beg + tid < nxt.end;
         if (has_nx) q_nx = rec[nxt.beg + tid];
@@ -861,7 +877,9 @@ __global__ void __launch_bounds__(GT) gather_kernel(CicGeom g, const uint4 *__re
         uint4 q2 = make_uint4(0, 0, 0, 0);
         if (tid + GT < cnt) q2 = rec[cur.beg + tid + GT];
         cp_async_wait<GST - 1>();  // this thread's copies of the current tile have landed ...
+        PM_STAMP(2);
         __syncthreads();     // ... and everybody else's
+        PM_STAMP(3);
         PIn pin2;
         if (tid + GT < cnt) pin2.load(q2.w, cot, ka);
 
@@ -961,17 +979,27 @@ __global__ void __launch_bounds__(GT) gather_kernel(CicGeom g, const uint4 *__re
                 }
             }
         }
+        PM_STAMP(4);
         // the next tile's first record has arrived by now: its per-particle inputs are requested before the barrier
         q = q_nx;
         if (has_nx) pin.load(q.w, cot, ka);
-        if (tid == 0) {
-            draw_publish(slot[(n + PUB) & 7]);
-            draw_request();
+        PM_STAMP(7);
+        if (tid == DRAWER) {
+            draw_publish(slot[(n + PUB) & 7], Spub);
+            PM_STAMP(8);
+            draw_request(Sfill, a_use, a_new);
         }
+        PM_STAMP(5);
         __syncthreads();  // stage n % GST may be overwritten; slot[(n + PUB) & 7] is published
+        PM_STAMP(6);
+        return true;
+    };
+    for (int n = 0;; n += 2) {
+        if (!body(n, S0, S1, a0, a1)) break;
+        if (!body(n + 1, S1, S0, a1, a0)) break;
     }
     cp_async_wait<0>();
-    if (tid == 0) sched_finish(g.sched);
+    if (tid == DRAWER) sched_finish(g.sched);
 }
 
 // --------------------------------------------------------------------------------------------------
