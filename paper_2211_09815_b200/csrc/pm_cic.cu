@@ -673,7 +673,7 @@ __global__ void __launch_bounds__(NTHREADS) scatter_kernel(const __grid_constant
 // two-stage cp.async pipeline: every thread first starts the copies of the NEXT tile's halo, then interpolates
 // for the particles of the current one.
 enum GatherMode { G_VALUE = 0, G_GRAD = 1, G_FUSED = 2 };
-constexpr int GT = 320;                                    // threads of a gather CTA
+constexpr int GT = 256;                                    // threads of a gather CTA
 constexpr int GCH = HZP / 4;                               // 16-byte pieces per halo row (9)
 constexpr int GRG = GT / GCH;                              // halo rows covered per pass of the CTA (28)
 
