@@ -48,6 +48,7 @@ struct CicGeom {
                    // int -> fp32 conversion (0 = plain density; nbar on the force path, whose k = 0 mode is zeroed
                    // anyway, so that fp32 rounding is relative to the fluctuation rho - nbar, not to rho)
     long long *dbgbuf;  // debug timeline (PM_DEBUG_CIC & 8): clock64 stamps of CTA 0
+    int sh1, sh2;  // log2 of nt[1], nt[2] when they are powers of two (tile index -> coordinates without a division), else -1
     int *sched;    // [0] tile counter, [1] finished CTAs; both zero between launches (the last CTA resets them)
 };
 
@@ -189,6 +190,11 @@ static CicGeom make_cic_geom(pm_ctx *c, const float *mesh, int C, int zs, long l
     { const char *e = getenv("PM_DEBUG_TMA_HALO"); r.tma_halo = e ? atoi(e) : 0; }
     { const char *e = getenv("PM_DEBUG_CIC"); r.dbg = e ? atoi(e) : 0; }
     r.sched = c->sched;
+    r.sh1 = r.sh2 = -1;
+    for (int k = 0; k < 31; k++) {
+        if (g.nt[1] == (1 << k)) r.sh1 = k;
+        if (g.nt[2] == (1 << k)) r.sh2 = k;
+    }
     r.dbgbuf = reinterpret_cast<long long *>(c->scal);
     memset(map, 0, sizeof(*map));
     long long off = mesh - c->mesh[0];
@@ -208,10 +214,17 @@ static CicGeom make_cic_geom(pm_ctx *c, const float *mesh, int C, int zs, long l
 // ---- tiles and scheduling -----------------------------------------------------------------------------
 __device__ __forceinline__ void tile_coords(const CicGeom &g, int tile, int t[3], int t0[3], int ext[3])
 {
-    t[2] = tile % g.nt[2];
-    const int r = tile / g.nt[2];
-    t[1] = r % g.nt[1];
-    t[0] = r / g.nt[1];
+    if (g.sh1 >= 0 && g.sh2 >= 0) {
+        t[2] = tile & (g.nt[2] - 1);
+        const int r = tile >> g.sh2;
+        t[1] = r & (g.nt[1] - 1);
+        t[0] = r >> g.sh1;
+    } else {
+        t[2] = tile % g.nt[2];
+        const int r = tile / g.nt[2];
+        t[1] = r % g.nt[1];
+        t[0] = r / g.nt[1];
+    }
     t0[0] = t[0] * TX; t0[1] = t[1] * TY; t0[2] = t[2] * TZ;
     ext[0] = min(TX, g.N[0] - t0[0]);
     ext[1] = min(TY, g.N[1] - t0[1]);
@@ -339,10 +352,6 @@ struct ScatterSlot {
     int n0;                     // leading records of the tile's own class 0 (all corners inside)
     int run_start[NRUNS];       // rec index = run_start[r] + flat index
     int run_prefix[NRUNS + 1];
-    int t0[3], ext[3];          // first mesh point and extent of the tile (computed once, by the producer)
-    float scale, inv_scale;     // unit-mass fixed-point scale of the tile
-    float mrest;                // mean subtraction: sub-quantum rest ...
-    long long mq;               // ... and whole quanta
 };
 
 // record stages: 4 for the scalar scatter (48 KB per CTA), 2 for three components (64 KB: three CTAs per SM)
@@ -401,20 +410,21 @@ __global__ void __launch_bounds__(NTHREADS) scatter_kernel(const __grid_constant
                 }
             }
         };
+        // Two register sets used by alternate iterations (the loop body is instantiated twice): the run lookup of tile
+        // n + 2 is requested at the end of iteration n into the set iteration n has just finished with, so every lookup
+        // has a whole iteration to complete and no value in flight is copied at the loop's back edge.
         TileDraw draw;
         if (lane == 0) draw.init(g.sched);
-        int tile = 0;
-        if (lane == 0) tile = draw.next(g.sched);
-        tile = __shfl_sync(0xffffffffu, tile, 0);
-        int b, len, n0;
-        lookup(tile, b, len, n0);
-        for (int n = 0;; n++) {
-            int tile_nx = 0;
-            if (lane == 0) tile_nx = draw.next(g.sched);
-            tile_nx = __shfl_sync(0xffffffffu, tile_nx, 0);
-            int b_nx, len_nx, n0_nx;
-            lookup(tile_nx, b_nx, len_nx, n0_nx);
-
+        auto draw_lookup = [&](int &tile, int &b, int &len, int &n0) {
+            int t = 0;
+            if (lane == 0) t = draw.next(g.sched);
+            tile = __shfl_sync(0xffffffffu, t, 0);
+            lookup(tile, b, len, n0);
+        };
+        int tileA, bA, lenA, n0A, tileB, bB, lenB, n0B;
+        draw_lookup(tileA, bA, lenA, n0A);
+        draw_lookup(tileB, bB, lenB, n0B);
+        auto body = [&](const int n, int &tile, int &b, int &len, int &n0) -> bool {
             const int s = n % NST;
             mbar_wait(&empty[s], ((n / NST) & 1) ^ 1);
             if (tile >= g.ntiles) {
@@ -423,7 +433,7 @@ __global__ void __launch_bounds__(NTHREADS) scatter_kernel(const __grid_constant
                     sched_finish(g.sched);
                 }
                 mbar_arrive(&full[s]);
-                break;
+                return false;
             }
             int inc = len;
 #pragma unroll
@@ -443,30 +453,6 @@ __global__ void __launch_bounds__(NTHREADS) scatter_kernel(const __grid_constant
                 slot[s].tile = tile;
                 slot[s].total = total;
                 slot[s].n0 = n0;
-                {
-                    int tt[3], tt0[3], text[3];
-                    tile_coords(g, tile, tt, tt0, text);
-#pragma unroll
-                    for (int d = 0; d < 3; d++) { slot[s].t0[d] = tt0[d]; slot[s].ext[d] = text[d]; }
-                    // unit mass: deposits are >= 0 -> UNSIGNED accumulation with scale = (2^32 - headroom) / total.  total is
-                    // an integer, so the scale is the same in every run: the density mesh stays bit-reproducible.  No point
-                    // can overflow: sum of weights at a point <= total, and each of the <= total deposits rounds by <= 0.5.
-                    const float room = fmaxf(4294967296.f * 0.99999f - (float)total, 1.f);
-                    const float sc = ldexpf(room / fmaxf((float)total, 1.f), -g.kshift);
-                    const float isc = 1.f / sc;
-                    slot[s].scale = sc;
-                    slot[s].inv_scale = isc;
-                    // mean subtraction (unit mass): mq quanta are removed exactly in integer, the sub-quantum rest in fp32
-                    long long mq = 0;
-                    float mrest = 0.f;
-                    if (g.mean != 0.0) {
-                        const double m = g.mean * (double)sc;
-                        mq = __double2ll_rn(m);
-                        mrest = (float)((m - (double)mq) * (double)isc);
-                    }
-                    slot[s].mq = mq;
-                    slot[s].mrest = mrest;
-                }
                 // the tile's own run: one bulk copy; the (short) neighbour runs: 16-byte async copies, one lane per run
                 if (cnt > 0) {
                     mbar_expect_tx(&full[s], (unsigned)cnt * (unsigned)sizeof(uint4));
@@ -478,7 +464,12 @@ __global__ void __launch_bounds__(NTHREADS) scatter_kernel(const __grid_constant
                 for (int k = 0; k < cnt; k++) cp_async16(&recbuf[s][start + k], rec + b + k);
                 cp_async_arrive(&full[s]);
             }
-            tile = tile_nx; b = b_nx; len = len_nx; n0 = n0_nx;
+            draw_lookup(tile, b, len, n0);  // for iteration n + 2
+            return true;
+        };
+        for (int n = 0;; n += 2) {
+            if (!body(n, tileA, bA, lenA, n0A)) break;
+            if (!body(n + 1, tileB, bB, lenB, n0B)) break;
         }
         return;
     }
@@ -495,12 +486,16 @@ __global__ void __launch_bounds__(NTHREADS) scatter_kernel(const __grid_constant
 
     for (int n = 0;; n++) {
         const int s = n % NST, b = n & 1;
+#define PM_SSTAMP(k) do { if ((g.dbg & 8) && blockIdx.x == 0 && n < 40 && (tid == 0 || tid == NCT - 1)) g.dbgbuf[((tid ? 1 : 0) * 40 + n) * 12 + (k)] = clock64(); } while (0)
+        PM_SSTAMP(0);
         mbar_wait(&full[s], (n / NST) & 1);
+        PM_SSTAMP(1);
         const ScatterSlot &sl = slot[s];
         const int tile = sl.tile;
         if (tile < 0) break;
         const int total = sl.total, n0 = sl.n0;
-        const int t0[3] = {sl.t0[0], sl.t0[1], sl.t0[2]}, ext[3] = {sl.ext[0], sl.ext[1], sl.ext[2]};
+        int t[3], t0[3], ext[3];
+        tile_coords(g, tile, t, t0, ext);
 
         // flat index -> record: the first RCAP are staged in shared memory, the rest come from global
         auto fetch = [&](int i) -> uint4 {
@@ -517,7 +512,12 @@ __global__ void __launch_bounds__(NTHREADS) scatter_kernel(const __grid_constant
 
         float scale;
         if (!HAS_VAL) {
-            scale = sl.scale;  // unit mass: computed by the producer (see there)
+            // unit mass: deposits are >= 0 -> UNSIGNED accumulation with scale = (2^32 - headroom) / total.  total is an
+            // integer, so the scale is the same in every run: the density mesh stays bit-reproducible.  No point can
+            // overflow: sum of weights at a point <= total, and each of the <= total deposits rounds by <= 0.5.
+            const float room = fmaxf(4294967296.f * 0.99999f - (float)total, 1.f);
+            scale = room / fmaxf((float)total, 1.f);
+            if (g.kshift) scale = ldexpf(scale, -g.kshift);
             for (int i = tid; i < total; i += NCT) {
                 const uint4 q = fetch(i);
                 if (i < n0) {
@@ -612,12 +612,22 @@ __global__ void __launch_bounds__(NTHREADS) scatter_kernel(const __grid_constant
                 }
             }
         }
-        const float inv_scale = HAS_VAL ? 1.f / scale : sl.inv_scale;
-        const long long mq = HAS_VAL ? 0ll : sl.mq;
-        const float mrest = HAS_VAL ? 0.f : sl.mrest;
+        const float inv_scale = 1.f / scale;
+        // mean subtraction (unit mass): mq quanta are removed exactly in integer, the sub-quantum rest in fp32
+        long long mq = 0;
+        float mrest = 0.f;
+        if (!HAS_VAL && g.mean != 0.0) {
+            const double m = g.mean * (double)scale;
+            mq = __double2ll_rn(m);
+            mrest = (float)((m - (double)mq) * (double)inv_scale);
+        }
 
+        PM_SSTAMP(2);
+        if ((g.dbg & 8) && blockIdx.x == 0 && n < 40 && tid == 0) g.dbgbuf[n * 12 + 11] = sl.total;
         if (tid == 0) tma_store_wait_read();  // the previous tile's store has read the other buffer out
+        PM_SSTAMP(3);
         consumer_sync();                      // all deposits of this tile are in; the other buffer is free
+        PM_SSTAMP(4);
         if (lane == 0) mbar_arrive(&empty[s]);
         {
             // int -> float in place (same bytes), and the other buffer is zeroed for the next tile
@@ -640,7 +650,9 @@ __global__ void __launch_bounds__(NTHREADS) scatter_kernel(const __grid_constant
             }
         }
         fence_proxy_async_smem();
+        PM_SSTAMP(5);
         consumer_sync();
+        PM_SSTAMP(6);
         if (g.use_tma) {
             if (tid == 0) {
 #pragma unroll
