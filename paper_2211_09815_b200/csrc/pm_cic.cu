@@ -48,6 +48,9 @@ struct CicGeom {
                    // int -> fp32 conversion (0 = plain density; nbar on the force path, whose k = 0 mode is zeroed
                    // anyway, so that fp32 rounding is relative to the fluctuation rho - nbar, not to rho)
     long long *dbgbuf;  // debug timeline (PM_DEBUG_CIC & 8): clock64 stamps of CTA 0
+    int *wq;       // gather overflow queue (pm_internal.cuh); items tagged with wq_epoch
+    int wq_cap;    // items the queue holds
+    unsigned wq_epoch;
     int sh1, sh2;  // log2 of nt[1], nt[2] when they are powers of two (tile index -> coordinates without a division), else -1
     int *sched;    // [0] tile counter, [1] finished CTAs; both zero between launches (the last CTA resets them)
 };
@@ -190,6 +193,9 @@ static CicGeom make_cic_geom(pm_ctx *c, const float *mesh, int C, int zs, long l
     { const char *e = getenv("PM_DEBUG_TMA_HALO"); r.tma_halo = e ? atoi(e) : 0; }
     { const char *e = getenv("PM_DEBUG_CIC"); r.dbg = e ? atoi(e) : 0; }
     r.sched = c->sched;
+    r.wq = c->wq;
+    r.wq_cap = (int)((c->wq_ints - 16) / 4);
+    r.wq_epoch = ++c->wq_epoch ? c->wq_epoch : ++c->wq_epoch;  // never 0 (the cleared buffer's tag)
     r.sh1 = r.sh2 = -1;
     for (int k = 0; k < 31; k++) {
         if (g.nt[1] == (1 << k)) r.sh1 = k;
@@ -255,12 +261,17 @@ struct TileDraw {
 };
 
 // called by one thread per CTA when it has drawn its last tile: the last CTA to finish re-arms the counters
-__device__ __forceinline__ void sched_finish(int *sched)
+__device__ __forceinline__ void sched_finish(int *sched, int *wq = nullptr)
 {
     __threadfence();
     if (atomicAdd(&sched[1], 1) == (int)gridDim.x - 1) {
         sched[0] = 0;
         sched[1] = 0;
+        if (wq) {
+            wq[0] = 0;
+            wq[1] = 0;
+            wq[2] = 0;
+        }
         __threadfence();
     }
 }
@@ -828,15 +839,66 @@ __global__ void __launch_bounds__(GT) gather_kernel(CicGeom g, const uint4 *__re
         }
         a_new = atomicAdd(&g.sched[0], 1);
     };
-    auto draw_publish = [&](GatherSlot &dst, const DrawSet &d) {
-        dst.tile = d.tile < g.ntiles ? d.tile : -1;
-        dst.beg = d.beg;
-        dst.end = d.end;
-        if (d.tile < g.ntiles) {
-            int tt[3], tt0[3], text[3];
-            tile_coords(g, d.tile, tt, tt0, text);
+    // Publishing a drawn tile.  A tile with more than GCHUNK particles is split: the first chunk is published, the others
+    // go to a global queue from which any CTA takes them once the tile counter is exhausted (a dense clump would
+    // otherwise keep one CTA busy long after all others have finished).  A pusher reserves its items with one atomic on
+    // the tail, writes them and tags them with this launch's epoch; a popper advances the head by compare-and-swap, so
+    // the head never passes the tail and an item pushed late is still found by whoever is alive (at least its pusher).
+    bool draw_done = false;  // drawing thread only
+    auto publish_range = [&](GatherSlot &dst, int tile, int beg, int end) {
+        dst.tile = tile;
+        dst.beg = beg;
+        dst.end = end;
+        int tt[3], tt0[3], text[3];
+        tile_coords(g, tile, tt, tt0, text);
 #pragma unroll
-            for (int k = 0; k < 3; k++) { dst.t0[k] = tt0[k]; dst.ext[k] = text[k]; }
+        for (int k = 0; k < 3; k++) { dst.t0[k] = tt0[k]; dst.ext[k] = text[k]; }
+    };
+    auto draw_publish = [&](GatherSlot &dst, const DrawSet &d) {
+        if (d.tile < g.ntiles) {
+            int end = d.end;
+            if (end - d.beg > GCHUNK) {
+                const int k = (end - d.beg + GCHUNK - 1) / GCHUNK - 1;
+                const int base = atomicAdd(&g.wq[1], k);
+                if (base + k <= g.wq_cap) {
+                    for (int i = 0; i < k; i++) {
+                        int *it = g.wq + 16 + 4 * (base + i);
+                        it[0] = d.tile;
+                        it[1] = d.beg + GCHUNK * (i + 1);
+                        it[2] = min(d.end, d.beg + GCHUNK * (i + 2));
+                    }
+                    __threadfence();
+                    for (int i = 0; i < k; i++) *reinterpret_cast<volatile unsigned *>(g.wq + 16 + 4 * (base + i) + 3) = g.wq_epoch;
+                    __threadfence();  // the tail update and the items are visible before this tile counts as published
+                    end = d.beg + GCHUNK;
+                } else {
+                    atomicSub(&g.wq[1], k);  // cannot happen with the sized queue; keep the tile whole
+                }
+            }
+            publish_range(dst, d.tile, d.beg, end);
+            atomicAdd(&g.wq[2], 1);  // one more tile whose chunks (if any) are in the queue (fenced above when it had any)
+            return;
+        }
+        // the tile counter is exhausted: take a chunk from the queue, or finish (and stay finished: the CTA stops at the
+        // first slot marked -1, so nothing may be taken from the queue after that).  The head is advanced by a plain
+        // fetch-and-add (a compare-and-swap loop collapses when hundreds of CTAs pop at once); an index beyond the tail
+        // waits until either an item is pushed there or every tile has been published (wq[2] == ntiles: no more pushes).
+        if (draw_done) { dst.tile = -1; return; }
+        const int idx = atomicAdd(&g.wq[0], 1);
+        for (;;) {
+            int t = *reinterpret_cast<volatile int *>(&g.wq[1]);
+            if (idx >= t && *reinterpret_cast<volatile int *>(&g.wq[2]) == g.ntiles) {
+                __threadfence();
+                t = *reinterpret_cast<volatile int *>(&g.wq[1]);
+                if (idx >= t) { draw_done = true; dst.tile = -1; return; }
+            }
+            if (idx < t) {
+                int *it = g.wq + 16 + 4 * idx;
+                while (*reinterpret_cast<volatile unsigned *>(it + 3) != g.wq_epoch) {}
+                __threadfence();
+                publish_range(dst, *reinterpret_cast<volatile int *>(it), *reinterpret_cast<volatile int *>(it + 1), *reinterpret_cast<volatile int *>(it + 2));
+                return;
+            }
         }
     };
     if (tid == DRAWER) {
@@ -1011,7 +1073,7 @@ __global__ void __launch_bounds__(GT) gather_kernel(CicGeom g, const uint4 *__re
         if (!body(n + 1, S1, S0, a1, a0)) break;
     }
     cp_async_wait<0>();
-    if (tid == DRAWER) sched_finish(g.sched);
+    if (tid == DRAWER) sched_finish(g.sched, g.wq);
 }
 
 // --------------------------------------------------------------------------------------------------

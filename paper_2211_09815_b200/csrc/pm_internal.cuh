@@ -19,6 +19,7 @@ namespace pm {
 // the LAST cell layer of the tile along x/y/z, i.e. when its CIC cloud reaches into the next tile.
 constexpr int TX = 8, TY = 8, TZ = 32;
 constexpr int NCLS = 8;
+constexpr int GCHUNK = 1024;  // gather: tiles with more particles are split into chunks that any CTA may take
 constexpr int PBITS = 36;  // momentum fixed point: p_fix = p * 2^PBITS (int64)
 constexpr int XBITS = 32;  // position fixed point: x_fix = (q + s) * 2^XBITS (int64, absolute, not wrapped)
 
@@ -93,6 +94,9 @@ struct pm_ctx {
     unsigned int scan_epoch;
     int *sched;                  // 2 ints: tile counter and finished-CTA count of the persistent CIC kernels (zero between launches)
     int num_sms;
+    int *wq;                     // overflow work queue of the gathers (chunks of heavy tiles): [0] head, [1] tail, items from [16]
+    long long wq_ints;           // ints per queue (two queues: one per stream)
+    unsigned int wq_epoch;       // tag of the items pushed by the current launch
     long long *x;                // [np][3] int64 absolute position (q + s) * 2^XBITS, not wrapped
     long long *p;                // [np][3] int64 momentum * 2^PBITS
     float *acc, *xi, *pi, *alpha;  // [np][3]
