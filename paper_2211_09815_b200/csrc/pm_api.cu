@@ -137,8 +137,10 @@ static size_t carve_workspace(pm_ctx *c, const Geometry &g, void *base)
     int *cursor = w.take<int>((size_t)g.nkeys + 1);
     int *hist = w.take<int>((size_t)g.nkeys + 1);
     int *sched = w.take<int>(64);
-    const long long wq_ints = 16 + 4 * ((long long)g.np / GCHUNK + g.ntiles + 64);
+    const long long wq_ints = 16 + 8 * ((long long)g.np / GCHUNK + g.ntiles + 64);
     int *wq = w.take<int>((size_t)(2 * wq_ints));
+    int *spool_ctl = w.take<int>(16 + 1024);
+    unsigned *spool = w.take<unsigned>((size_t)1024 * TX * TY * TZ);
     unsigned long long *scan_agg = w.take<unsigned long long>((size_t)(g.nkeys + 1) / 4096 + 2);
     long long *x = w.take<long long>((size_t)g.np * 3);
     long long *p = w.take<long long>((size_t)g.np * 3);
@@ -154,7 +156,7 @@ static size_t carve_workspace(pm_ctx *c, const Geometry &g, void *base)
     void *fftw = w.take<char>(fft_work_reserve(g));
     if (c) {
         for (int k = 0; k < 7; k++) c->mesh[k] = m + (size_t)k * g.mesh_stride;
-        c->rec = rec; c->offsets = offsets; c->cursor = cursor; c->hist = hist; c->sched = sched; c->wq = wq; c->wq_ints = wq_ints; c->scan_agg = scan_agg;
+        c->rec = rec; c->offsets = offsets; c->cursor = cursor; c->hist = hist; c->sched = sched; c->wq = wq; c->wq_ints = wq_ints; c->spool_ctl = spool_ctl; c->spool = spool; c->scan_agg = scan_agg;
         c->x = x; c->p = p; c->acc = acc; c->xi = xi; c->pi = pi; c->alpha = alpha;
         c->scal = scal; c->ktab = ktab; c->ktabn = tabn;
         c->fft_tab = ffttab;
@@ -326,6 +328,9 @@ int pm_init(pm_ctx **out, const pm_params *params, void *dev_workspace, size_t b
     c->scan_epoch = 0;
     c->wq_epoch = 0;
     if (rc == PM_OK && cudaMemsetAsync(c->wq, 0, sizeof(int) * (size_t)(2 * c->wq_ints), c->stream) != cudaSuccess) rc = fail(c, PM_ECUDA, "pm_init", "clearing the gather work queue");
+    if (rc == PM_OK && (cudaMemsetAsync(c->spool_ctl, 0, sizeof(int) * (16 + 1024), c->stream) != cudaSuccess ||
+                        cudaMemsetAsync(c->spool, 0, sizeof(unsigned) * (size_t)1024 * TX * TY * TZ, c->stream) != cudaSuccess))
+        rc = fail(c, PM_ECUDA, "pm_init", "clearing the scatter accumulator pool");
     c->overlap_ok = false;
     {
         const char *e = getenv("PM_OVERLAP");

@@ -48,6 +48,8 @@ struct CicGeom {
                    // int -> fp32 conversion (0 = plain density; nbar on the force path, whose k = 0 mode is zeroed
                    // anyway, so that fp32 rounding is relative to the fluctuation rho - nbar, not to rho)
     long long *dbgbuf;  // debug timeline (PM_DEBUG_CIC & 8): clock64 stamps of CTA 0
+    int *spool_ctl;     // scatter pool: [0] next free accumulator, [16 + p] chunks of accumulator p that have arrived
+    unsigned *spool;    // scatter pool: SPOOL_N accumulators of TILE_PTS uint32, all zero between uses
     int *wq;       // gather overflow queue (pm_internal.cuh); items tagged with wq_epoch
     int wq_cap;    // items the queue holds
     unsigned wq_epoch;
@@ -63,6 +65,8 @@ constexpr int HALO_STRIDE = (HALO_PTS + 31) / 32 * 32;    // per-mesh stride in 
 constexpr int NCW = 8;                                    // consumer warps
 constexpr int NCT = NCW * 32;                             // consumer threads
 constexpr int NTHREADS = NCT + 32;                        // + one producer warp
+constexpr int SCHUNK = 2048;                               // scatter: records per chunk of a heavy tile
+constexpr int SPOOL_N = 1024;                              // scatter: global accumulators for heavy tiles (8 KB each)
 constexpr int RCAP = 512;                                 // records staged in shared memory per tile (the rest are read from global)
 
 // ---- PTX wrappers: mbarrier + TMA (sm_90+/sm_100a) ----------------------------------------------------
@@ -194,7 +198,9 @@ static CicGeom make_cic_geom(pm_ctx *c, const float *mesh, int C, int zs, long l
     { const char *e = getenv("PM_DEBUG_CIC"); r.dbg = e ? atoi(e) : 0; }
     r.sched = c->sched;
     r.wq = c->wq;
-    r.wq_cap = (int)((c->wq_ints - 16) / 4);
+    r.wq_cap = (int)((c->wq_ints - 16) / (store ? 8 : 4));  // scatter items are 8 ints, gather items 4
+    r.spool_ctl = c->spool_ctl;
+    r.spool = c->spool;
     r.wq_epoch = ++c->wq_epoch ? c->wq_epoch : ++c->wq_epoch;  // never 0 (the cleared buffer's tag)
     r.sh1 = r.sh2 = -1;
     for (int k = 0; k < 31; k++) {
@@ -261,7 +267,7 @@ struct TileDraw {
 };
 
 // called by one thread per CTA when it has drawn its last tile: the last CTA to finish re-arms the counters
-__device__ __forceinline__ void sched_finish(int *sched, int *wq = nullptr)
+__device__ __forceinline__ void sched_finish(int *sched, int *wq = nullptr, int *spool_ctl = nullptr)
 {
     __threadfence();
     if (atomicAdd(&sched[1], 1) == (int)gridDim.x - 1) {
@@ -272,6 +278,7 @@ __device__ __forceinline__ void sched_finish(int *sched, int *wq = nullptr)
             wq[1] = 0;
             wq[2] = 0;
         }
+        if (spool_ctl) spool_ctl[0] = 0;
         __threadfence();
     }
 }
@@ -363,6 +370,8 @@ struct ScatterSlot {
     int n0;                     // leading records of the tile's own class 0 (all corners inside)
     int run_start[NRUNS];       // rec index = run_start[r] + flat index
     int run_prefix[NRUNS + 1];
+    int lo, hi;                 // flat record range of this work item: [0, total) or one chunk of a heavy tile
+    int pool;                   // heavy tile: slot of the global integer accumulator the chunks are combined in; else -1
 };
 
 // record stages: 4 for the scalar scatter (48 KB per CTA), 2 for three components (64 KB: three CTAs per SM)
@@ -385,6 +394,7 @@ __global__ void __launch_bounds__(NTHREADS) scatter_kernel(const __grid_constant
     __shared__ __align__(8) unsigned long long full[NST], empty[NST];
     __shared__ ScatterSlot slot[NST];
     __shared__ float redf[NCW];
+    __shared__ int heavy_last;
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (threadIdx.x == 0) {
@@ -435,47 +445,133 @@ __global__ void __launch_bounds__(NTHREADS) scatter_kernel(const __grid_constant
         int tileA, bA, lenA, n0A, tileB, bB, lenB, n0B;
         draw_lookup(tileA, bA, lenA, n0A);
         draw_lookup(tileB, bB, lenB, n0B);
-        auto body = [&](const int n, int &tile, int &b, int &len, int &n0) -> bool {
-            const int s = n % NST;
-            mbar_wait(&empty[s], ((n / NST) & 1) ^ 1);
-            if (tile >= g.ntiles) {
-                if (lane == 0) {
-                    slot[s].tile = -1;
-                    sched_finish(g.sched);
-                }
-                mbar_arrive(&full[s]);
-                return false;
-            }
-            int inc = len;
+        // publishes one work item into stage s: run table, flat range [lo, hi) and the staged records of that range
+        // inclusive prefix of the run lengths over the lanes; returns the total
+        auto run_scan = [&](int len, int &inc) {
+            inc = len;
 #pragma unroll
             for (int o = 1; o < 16; o <<= 1) {
                 const int u = __shfl_up_sync(0xffffffffu, inc, o);
                 if (lane >= o) inc += u;
             }
+            return __shfl_sync(0xffffffffu, inc, NRUNS - 1);
+        };
+        auto publish = [&](int s, int tile, int b, int len, int inc, int total, int n0, int lo, int hi, int pool) {
             const int start = inc - len;
-            const int total = __shfl_sync(0xffffffffu, inc, NRUNS - 1);
+            if (hi < 0) hi = total;
             if (lane < NRUNS) {
                 slot[s].run_start[lane] = b - start;
                 slot[s].run_prefix[lane + 1] = inc;
             }
-            const int cnt = lane < NRUNS ? max(min(len, RCAP - start), 0) : 0;
+            // this lane's run restricted to [lo, min(hi, lo + RCAP)): staged at recbuf[flat - lo]
+            const int s0 = max(start, lo), e0 = min(min(start + len, hi), lo + RCAP);
+            const int cnt = lane < NRUNS ? max(e0 - s0, 0) : 0;
             if (lane == 0) {
                 slot[s].run_prefix[0] = 0;
                 slot[s].tile = tile;
                 slot[s].total = total;
                 slot[s].n0 = n0;
+                slot[s].lo = lo;
+                slot[s].hi = hi;
+                slot[s].pool = pool;
                 // the tile's own run: one bulk copy; the (short) neighbour runs: 16-byte async copies, one lane per run
                 if (cnt > 0) {
                     mbar_expect_tx(&full[s], (unsigned)cnt * (unsigned)sizeof(uint4));
-                    bulk_load(&recbuf[s][0], rec + b, (unsigned)cnt * (unsigned)sizeof(uint4), &full[s]);
+                    bulk_load(&recbuf[s][s0 - lo], rec + b + (s0 - start), (unsigned)cnt * (unsigned)sizeof(uint4), &full[s]);
                 } else {
                     mbar_arrive(&full[s]);
                 }
             } else {
-                for (int k = 0; k < cnt; k++) cp_async16(&recbuf[s][start + k], rec + b + k);
+                for (int k = 0; k < cnt; k++) cp_async16(&recbuf[s][s0 - lo + k], rec + b + (s0 - start) + k);
                 cp_async_arrive(&full[s]);
             }
-            draw_lookup(tile, b, len, n0);  // for iteration n + 2
+        };
+        bool draw_done = false;
+        auto body = [&](const int n, int &tile, int &b, int &len, int &n0) -> bool {
+            const int s = n % NST;
+            mbar_wait(&empty[s], ((n / NST) & 1) ^ 1);
+            if (tile < g.ntiles) {
+                // A heavy tile (unit mass only) is split into chunks of SCHUNK records that any CTA may take from the global
+                // queue; the chunks add their integer accumulators into one global accumulator of the pool (same scale:
+                // it depends on the tile's total only), and the last chunk to arrive converts and stores the tile.
+                int inc;
+                const int total = run_scan(len, inc);
+                int lo = 0, hi = -1, pool = -1;
+                if (!HAS_VAL && C == 1 && total > SCHUNK + SCHUNK / 2) {
+                    const int k = (total + SCHUNK - 1) / SCHUNK;
+                    int base = 0;
+                    if (lane == 0) {
+                        pool = atomicAdd(&g.spool_ctl[0], 1);
+                        if (pool < SPOOL_N) {
+                            base = atomicAdd(&g.wq[1], k - 1);
+                            if (base + k - 1 > g.wq_cap) { atomicSub(&g.wq[1], k - 1); pool = -1; }
+                        } else {
+                            pool = -1;
+                        }
+                    }
+                    pool = __shfl_sync(0xffffffffu, pool, 0);
+                    base = __shfl_sync(0xffffffffu, base, 0);
+                    if (pool >= 0) {
+                        for (int i = lane; i < k - 1; i += 32) {
+                            int *it = g.wq + 16 + 8 * (base + i);
+                            it[0] = tile;
+                            it[1] = SCHUNK * (i + 1);
+                            it[2] = min(total, SCHUNK * (i + 2));
+                            it[3] = pool;
+                        }
+                        __threadfence();
+                        __syncwarp();
+                        for (int i = lane; i < k - 1; i += 32) *reinterpret_cast<volatile unsigned *>(g.wq + 16 + 8 * (base + i) + 4) = g.wq_epoch;
+                        __threadfence();
+                        hi = SCHUNK;
+                    }
+                }
+                publish(s, tile, b, len, inc, total, n0, lo, hi, pool);
+                if (lane == 0) atomicAdd(&g.wq[2], 1);  // one more tile whose chunks (if any) are in the queue
+                draw_lookup(tile, b, len, n0);  // for iteration n + 2
+                return true;
+            }
+            // the tile counter is exhausted: chunks from the queue (fetch-and-add head; see the gather kernel), then finish
+            int it_tile = -1, it_lo = 0, it_hi = 0, it_pool = -1;
+            if (lane == 0 && !draw_done) {
+                const int idx = atomicAdd(&g.wq[0], 1);
+                for (;;) {
+                    int t = *reinterpret_cast<volatile int *>(&g.wq[1]);
+                    if (idx >= t && *reinterpret_cast<volatile int *>(&g.wq[2]) == g.ntiles) {
+                        __threadfence();
+                        t = *reinterpret_cast<volatile int *>(&g.wq[1]);
+                        if (idx >= t) break;
+                    }
+                    if (idx < t) {
+                        int *it = g.wq + 16 + 8 * idx;
+                        while (*reinterpret_cast<volatile unsigned *>(it + 4) != g.wq_epoch) {}
+                        __threadfence();
+                        it_tile = *reinterpret_cast<volatile int *>(it);
+                        it_lo = *reinterpret_cast<volatile int *>(it + 1);
+                        it_hi = *reinterpret_cast<volatile int *>(it + 2);
+                        it_pool = *reinterpret_cast<volatile int *>(it + 3);
+                        break;
+                    }
+                }
+            }
+            it_tile = __shfl_sync(0xffffffffu, it_tile, 0);
+            if (it_tile < 0) {
+                draw_done = true;
+                if (lane == 0) {
+                    slot[s].tile = -1;
+                    sched_finish(g.sched, g.wq, (!HAS_VAL && C == 1) ? g.spool_ctl : nullptr);
+                }
+                mbar_arrive(&full[s]);
+                return false;
+            }
+            it_lo = __shfl_sync(0xffffffffu, it_lo, 0);
+            it_hi = __shfl_sync(0xffffffffu, it_hi, 0);
+            it_pool = __shfl_sync(0xffffffffu, it_pool, 0);
+            int qb, qlen, qn0;
+            lookup(it_tile, qb, qlen, qn0);
+            int qinc;
+            const int qtotal = run_scan(qlen, qinc);
+            publish(s, it_tile, qb, qlen, qinc, qtotal, qn0, it_lo, it_hi, it_pool);
             return true;
         };
         for (int n = 0;; n += 2) {
@@ -505,12 +601,13 @@ __global__ void __launch_bounds__(NTHREADS) scatter_kernel(const __grid_constant
         const int tile = sl.tile;
         if (tile < 0) break;
         const int total = sl.total, n0 = sl.n0;
+        const int lo = sl.lo, hi = sl.hi, pool = sl.pool;
         int t[3], t0[3], ext[3];
         tile_coords(g, tile, t, t0, ext);
 
-        // flat index -> record: the first RCAP are staged in shared memory, the rest come from global
+        // flat index -> record: the first RCAP of the range are staged in shared memory, the rest come from global
         auto fetch = [&](int i) -> uint4 {
-            if (i < RCAP) return recbuf[s][i];
+            if (i - lo < RCAP) return recbuf[s][i - lo];
             int r = 0;
             while (i >= sl.run_prefix[r + 1]) r++;
             return rec[sl.run_start[r] + i];
@@ -529,7 +626,7 @@ __global__ void __launch_bounds__(NTHREADS) scatter_kernel(const __grid_constant
             const float room = fmaxf(4294967296.f * 0.99999f - (float)total, 1.f);
             scale = room / fmaxf((float)total, 1.f);
             if (g.kshift) scale = ldexpf(scale, -g.kshift);
-            for (int i = tid; i < total; i += NCT) {
+            for (int i = lo + tid; i < hi; i += NCT) {
                 const uint4 q = fetch(i);
                 if (i < n0) {
                     Corners<true> cn(g, t0, ext, q, fr, fmask);
@@ -640,6 +737,31 @@ __global__ void __launch_bounds__(NTHREADS) scatter_kernel(const __grid_constant
         consumer_sync();                      // all deposits of this tile are in; the other buffer is free
         PM_SSTAMP(4);
         if (lane == 0) mbar_arrive(&empty[s]);
+        bool do_store = true;
+        if (!HAS_VAL && C == 1 && pool >= 0) {
+            // chunk of a heavy tile: add the accumulators into the tile's global accumulator (integers: the result does
+            // not depend on who adds first and equals what one CTA alone would have accumulated); the chunk that finds
+            // all others done takes the sums back, converts and stores them and leaves the accumulator zeroed
+            unsigned *gp = g.spool + (size_t)pool * TILE_PTS;
+            for (int i = tid; i < TILE_PTS; i += NCT) {
+                const unsigned v = (unsigned)tile_acc[i];
+                if (v) atomicAdd(gp + i, v);
+            }
+            __threadfence();
+            consumer_sync();
+            if (tid == 0) heavy_last = atomicAdd(&g.spool_ctl[16 + pool], 1) == (total + SCHUNK - 1) / SCHUNK - 1;
+            consumer_sync();
+            do_store = heavy_last != 0;
+            if (do_store) {
+                __threadfence();
+                for (int i = tid; i < TILE_PTS; i += NCT) {
+                    tile_acc[i] = (int)__ldcg(gp + i);
+                    gp[i] = 0u;
+                }
+                if (tid == 0) g.spool_ctl[16 + pool] = 0;
+            }
+            consumer_sync();
+        }
         {
             // int -> float in place (same bytes), and the other buffer is zeroed for the next tile
             int4 *a4 = reinterpret_cast<int4 *>(tile_acc);
@@ -664,7 +786,9 @@ __global__ void __launch_bounds__(NTHREADS) scatter_kernel(const __grid_constant
         PM_SSTAMP(5);
         consumer_sync();
         PM_SSTAMP(6);
-        if (g.use_tma) {
+        if (!do_store) {
+            // another chunk of this tile stores it
+        } else if (g.use_tma) {
             if (tid == 0) {
 #pragma unroll
                 for (int c = 0; c < C; c++) tma_store_4d(&tmap, tile_acc + c * TILE_PTS, t0[2], t0[1], t0[0], g.c0 + c);

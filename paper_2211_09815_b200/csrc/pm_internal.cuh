@@ -97,6 +97,8 @@ struct pm_ctx {
     int *wq;                     // overflow work queue of the gathers (chunks of heavy tiles): [0] head, [1] tail, items from [16]
     long long wq_ints;           // ints per queue (two queues: one per stream)
     unsigned int wq_epoch;       // tag of the items pushed by the current launch
+    int *spool_ctl;              // scatter pool control: [0] next accumulator, [16 + p] arrived chunks
+    unsigned *spool;             // scatter pool: 1024 accumulators of one tile (8 KB) each, zero between uses
     long long *x;                // [np][3] int64 absolute position (q + s) * 2^XBITS, not wrapped
     long long *p;                // [np][3] int64 momentum * 2^PBITS
     float *acc, *xi, *pi, *alpha;  // [np][3]
