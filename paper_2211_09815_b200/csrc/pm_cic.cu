@@ -41,7 +41,6 @@ struct CicGeom {
     int use_tma;   // tensor map valid for this mesh (16-byte aligned base and strides)
     int c0;        // first component (4th tensor-map coordinate)
     int dbg;       // debug bits (PM_DEBUG_CIC): 1 = gather skips the particle loop, 2 = gather skips the halo copies
-    int tma_halo;  // debug: 1 = interior halos by TMA tensor loads instead of 16-byte async copies (PM_DEBUG_TMA_HALO)
     int kshift;    // debug: coarsen the scatter's fixed-point scale by this many bits (0 in production)
     int ntiles;
     double mean;   // unit-mass scatter only: constant subtracted from every mesh point IN INTEGER, before the
@@ -191,11 +190,13 @@ static CicGeom make_cic_geom(pm_ctx *c, const float *mesh, int C, int zs, long l
     r.ms = ms;
     r.use_tma = 0;
     r.c0 = 0;
-    { const char *e = getenv("PM_DEBUG_KSHIFT"); r.kshift = e ? atoi(e) : 0; }
+    // debug knobs, read once per process
+    static const int env_kshift = [] { const char *e = getenv("PM_DEBUG_KSHIFT"); return e ? atoi(e) : 0; }();
+    static const int env_dbg = [] { const char *e = getenv("PM_DEBUG_CIC"); return e ? atoi(e) : 0; }();
+    r.kshift = env_kshift;
     r.mean = 0.0;
     r.ntiles = g.ntiles;
-    { const char *e = getenv("PM_DEBUG_TMA_HALO"); r.tma_halo = e ? atoi(e) : 0; }
-    { const char *e = getenv("PM_DEBUG_CIC"); r.dbg = e ? atoi(e) : 0; }
+    r.dbg = env_dbg;
     r.sched = c->sched;
     r.wq = c->wq;
     r.wq_cap = (int)((c->wq_ints - 16) / (store ? 8 : 4));  // scatter items are 8 ints, gather items 4
