@@ -38,7 +38,7 @@ struct CicGeom {
     int fbits;
     int zs;        // floats per z-row
     long long ms;  // floats per mesh (component stride)
-    int use_tma;   // tensor map valid for this mesh (16-byte aligned base and strides)
+    int use_tma;   // scatter: tensor map valid for this mesh; gather: base and strides are 16-byte aligned (async row copies)
     int c0;        // first component (4th tensor-map coordinate)
     int dbg;       // debug bits (PM_DEBUG_CIC): 1 = gather skips the particle loop, 2 = gather skips the halo copies
     int kshift;    // debug: coarsen the scatter's fixed-point scale by this many bits (0 in production)
@@ -174,8 +174,7 @@ static bool encode_mesh_map(CUtensorMap *out, const float *base, const int N[3],
 int cic_init_tensor_maps(pm_ctx *c)
 {
     const Geometry &g = c->g;
-    c->tma_ok = encode_mesh_map(&c->tmap_load, c->mesh[0], g.N, 7, g.zs, g.mesh_stride, HZP, HY, HX) &&
-                encode_mesh_map(&c->tmap_store, c->mesh[0], g.N, 7, g.zs, g.mesh_stride, TZ, TY, TX);
+    c->tma_ok = encode_mesh_map(&c->tmap_store, c->mesh[0], g.N, 7, g.zs, g.mesh_stride, TZ, TY, TX);
     return PM_OK;
 }
 
@@ -213,13 +212,15 @@ static CicGeom make_cic_geom(pm_ctx *c, const float *mesh, int C, int zs, long l
     long long off = mesh - c->mesh[0];
     bool internal = zs == g.zs && ms == g.mesh_stride && mesh >= c->mesh[0] && off % g.mesh_stride == 0 &&
                     off / g.mesh_stride + C <= 7;
-    if (internal && c->tma_ok) {
-        *map = store ? c->tmap_store : c->tmap_load;
+    if (!store) {
+        // gathers copy halo rows in 16-byte pieces: all they need is a 16-byte aligned base and strides (no tensor map)
+        r.use_tma = (((uintptr_t)mesh & 15) == 0 && (zs & 3) == 0 && (ms & 3) == 0) ? 1 : 0;
+    } else if (internal && c->tma_ok) {
+        *map = c->tmap_store;
         r.use_tma = 1;
         r.c0 = (int)(off / g.mesh_stride);
     } else if (!internal) {
-        if (store ? encode_mesh_map(map, mesh, g.N, C, zs, ms, TZ, TY, TX) : encode_mesh_map(map, mesh, g.N, C, zs, ms, HZP, HY, HX))
-            r.use_tma = 1;
+        if (encode_mesh_map(map, mesh, g.N, C, zs, ms, TZ, TY, TX)) r.use_tma = 1;
     }
     return r;
 }

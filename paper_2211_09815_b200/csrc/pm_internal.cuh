@@ -106,7 +106,7 @@ struct pm_ctx {
     double *ktab;                // [3 axes][3: kt, k^2, dec][ktabn] per-axis k-space tables (fp64)
     int ktabn;
     long long cur_np;            // particles in the current sort
-    CUtensorMap tmap_load, tmap_store;  // 4-D {z, y, x, mesh 0..6} views of the internal meshes: halo box / tile box
+    CUtensorMap tmap_store;      // 4-D {z, y, x, mesh 0..6} view of the internal meshes with the tile box (scatter stores)
     bool tma_ok;                 // cuTensorMapEncodeTiled resolved and the internal maps encoded
     void *fft_work;
     bool own_fft;                // power-of-two mesh: own FFT passes with the k-space operators fused (pm_fft.cu)
