@@ -79,7 +79,7 @@ int pm_host_growth(double omega_m, double a, double out[4]);
 int pm_host_step_factors(double omega_m, double a_prev, double a_next, double out[3]);
 /*   memory order of the library's own FFT passes along an axis of n points (n a power of two, 8 <= n <= 1024):
  *   out[p] = frequency index (0 .. n-1, e^{-2 pi i k g / n} convention) that memory position p holds after the
- *   forward decimation-in-frequency stages (radix 16, ..., then the remainder).  Pure host; the k-space tables are
+ *   forward decimation-in-frequency stages (radix 16, or 8 where a radix-2 stage would otherwise remain).  Pure host; the k-space tables are
  *   built from it and nothing in k-space crosses this ABI (R26). */
 int pm_host_fft_order(int32_t n, int32_t *out);
 /*   the factors stored in ctx for forward step i in 1..n; the adjoint step uses their exact negatives (L389) */

@@ -89,13 +89,22 @@ __device__ __forceinline__ void reg_dft(float2 (&v)[R])
 
 constexpr int FFT_T = 256;  // threads per CTA of every FFT kernel
 
+// radix of the stage that works on spans of length L (a power of two): 16 where possible, but 8 when that would leave a
+// radix-2 stage at the end (L = 32, 512, ...: 32 = 8 x 4, 512 = 8 x 16 x 4); the host mirror uses the same function
+__host__ __device__ constexpr int stage_radix(int L)
+{
+    int lg = 0;
+    for (int v = L; v > 1; v >>= 1) lg++;
+    return L >= 16 ? (lg % 4 == 1 ? 8 : 16) : L;
+}
+
 // ---- one transform along the tile's position axis, everything but the data known at compile time -----------
 // tile [N][PITCH] (float2), columns [0, ncol) of 1 << CS; tw = exp(-2 pi i k / N), k < N (shared memory).
-// Stage of span L, radix R = min(16, L): butterfly (blk, j) takes positions blk L + j + m L/R, m < R.
+// Stage of span L, radix R = stage_radix(L): butterfly (blk, j) takes positions blk L + j + m L/R, m < R.
 template <int N, int L, bool INV, int PITCH, int CS>
 __device__ __forceinline__ void fft_stage(float2 *tile, int ncol, const float2 *tw)
 {
-    constexpr int R = L >= 16 ? 16 : L;
+    constexpr int R = stage_radix(L);
     constexpr int Lr = L / R, twstep = N / L;
     constexpr int nwork = (N / R) << CS;
 #pragma unroll 1
@@ -125,7 +134,7 @@ __device__ __forceinline__ void fft_stage(float2 *tile, int ncol, const float2 *
 
 template <int N, int L, bool INV, int PITCH, int CS>
 struct AxisFFT {
-    static constexpr int R = L >= 16 ? 16 : L;
+    static constexpr int R = stage_radix(L);
     static __device__ __forceinline__ void run(float2 *tile, int ncol, const float2 *tw)
     {
         if (!INV) {
@@ -504,7 +513,7 @@ static AxisPlan make_axis_plan(int N)
     p.nst = 0;
     int n = N;
     while (n > 1) {
-        int r = n >= 16 ? 16 : n;  // 16, ..., then the remainder 8 / 4 / 2
+        int r = stage_radix(n);
         p.radix[p.nst] = r;
         p.span[p.nst] = n;
         p.nst++;

@@ -93,7 +93,7 @@ def test_host_growth_matches_oracle_ode(binding, orc, om):
 
 def test_own_fft_memory_order_is_the_dif_digit_reversal(binding):
     """pm_host_fft_order against an independent numpy run of the same in-place decimation-in-frequency schedule
-    (radix min(16, L) per stage, csrc/pm_fft.cu): position p of the staged result must hold numpy.fft.fft's bin out[p]."""
+    (radix 16 per stage, 8 where a radix-2 stage would otherwise remain, csrc/pm_fft.cu): position p of the staged result must hold numpy.fft.fft's bin out[p]."""
     rng = np.random.default_rng(3)
     for n in (8, 16, 32, 64, 128, 256, 512, 1024):
         order = np.asarray(binding.host_fft_order(n))
@@ -102,7 +102,7 @@ def test_own_fft_memory_order_is_the_dif_digit_reversal(binding):
         y = x.copy()
         L = n
         while L > 1:
-            R = min(16, L)
+            R = (8 if (L.bit_length() - 1) % 4 == 1 else 16) if L >= 16 else L
             Lr = L // R
             for blk in range(n // L):
                 for j in range(Lr):
