@@ -107,6 +107,16 @@ __device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned phas
         ::"r"(smem_u32(bar)), "r"(phase), "r"(20000u)
         : "memory");
 }
+// non-blocking: has the phase with this parity completed?
+__device__ __forceinline__ bool mbar_test(unsigned long long *bar, unsigned phase)
+{
+    unsigned ok;
+    asm volatile("{\n .reg .pred p;\n mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+                 : "=r"(ok)
+                 : "r"(smem_u32(bar)), "r"(phase)
+                 : "memory");
+    return ok != 0;
+}
 __device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *m, unsigned long long *bar, int z, int y, int x, int c)
 {
     asm volatile(
@@ -593,6 +603,12 @@ __global__ void __launch_bounds__(NTHREADS) scatter_kernel(const __grid_constant
     const float fr = 1.f / (float)(1u << g.fbits);
     const unsigned fmask = (1u << g.fbits) - 1u;
 
+    // valued scatter: records and values of the NEXT tile's first two rounds, requested while this tile is finished
+    bool pre_ok = false;
+    uint4 pqa = make_uint4(0, 0, 0, 0), pqb = pqa;
+    float pva[C], pvb[C];
+#pragma unroll
+    for (int c = 0; c < C; c++) pva[c] = pvb[c] = 0.f;
     for (int n = 0;; n++) {
         const int s = n % NST, b = n & 1;
 #define PM_SSTAMP(k) do { if ((g.dbg & 8) && blockIdx.x == 0 && n < 40 && (tid == 0 || tid == NCT - 1)) g.dbgbuf[((tid ? 1 : 0) * 40 + n) * 12 + (k)] = clock64(); } while (0)
@@ -648,8 +664,14 @@ __global__ void __launch_bounds__(NTHREADS) scatter_kernel(const __grid_constant
             float va[C], vb[C];
 #pragma unroll
             for (int c = 0; c < C; c++) va[c] = vb[c] = 0.f;
-            if (ia < total) { qa = fetch(ia); values(qa, va); }
-            if (ib < total) { qb = fetch(ib); values(qb, vb); }
+            if (pre_ok) {
+                qa = pqa; qb = pqb;
+#pragma unroll
+                for (int c = 0; c < C; c++) { va[c] = pva[c]; vb[c] = pvb[c]; }
+            } else {
+                if (ia < total) { qa = fetch(ia); values(qa, va); }
+                if (ib < total) { qb = fetch(ib); values(qb, vb); }
+            }
             float ma = 0.f, mb = 0.f;
 #pragma unroll
             for (int c = 0; c < C; c++) { ma = fmaxf(ma, fabsf(va[c])); mb = fmaxf(mb, fabsf(vb[c])); }
@@ -719,6 +741,28 @@ __global__ void __launch_bounds__(NTHREADS) scatter_kernel(const __grid_constant
                     float v[C];
                     values(q, v);
                     pass_b(i, q, v);
+                }
+            }
+        }
+        if (HAS_VAL) {
+            // if the producer has the next tile staged already, request its first two rounds of values now: their
+            // round trip then overlaps the conversion and the store of this tile
+            const int s1 = (n + 1) % NST;
+            pre_ok = mbar_test(&full[s1], ((n + 1) / NST) & 1) && slot[s1].tile >= 0 && slot[s1].pool < 0;
+            if (pre_ok) {
+                const int total1 = slot[s1].total;
+#pragma unroll
+                for (int c = 0; c < C; c++) pva[c] = pvb[c] = 0.f;
+                pqa = pqb = make_uint4(0, 0, 0, 0);
+                if (tid < total1) {
+                    pqa = recbuf[s1][tid];
+#pragma unroll
+                    for (int c = 0; c < C; c++) pva[c] = val[(size_t)pqa.w * C + c];
+                }
+                if (tid + NCT < total1) {
+                    pqb = recbuf[s1][tid + NCT];
+#pragma unroll
+                    for (int c = 0; c < C; c++) pvb[c] = val[(size_t)pqb.w * C + c];
                 }
             }
         }
