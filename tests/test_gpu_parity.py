@@ -99,6 +99,8 @@ def test_scatter_is_bit_reproducible_and_order_independent(pmlib):
     rng = np.random.default_rng(5)
     pm = pmlib.PM(mesh, lattice, 1.0, [0.5, 1.0])
     x = rand_positions(rng, pm.np, mesh, spread=0.0)
+    # a dense clump: its tile goes through the split path (chunks combined in a global integer accumulator)
+    x[: pm.np // 3] = (np.asarray(mesh) * 0.41 + rng.normal(0, 0.5, (pm.np // 3, 3))).astype(np.float32)
     a = pm.scatter(dev(x)).cpu().numpy()
     b = pm.scatter(dev(x)).cpu().numpy()
     c = pm.scatter(dev(x[rng.permutation(pm.np)])).cpu().numpy()
