@@ -142,10 +142,11 @@ int pm_run_fwd_adj(pm_ctx *ctx, const float *dev_s0, const float *dev_p0, const 
                    float *dev_s_n, float *dev_p_n, double *host_J, float *dev_xi0, float *dev_pi0,
                    float *dev_dJ_ds0, float *dev_s_rec, float *dev_p_rec);
 /* Same through HOST buffers: copies s0, p0, delta_target host->device, runs, copies every non-NULL
- * output device->host, synchronises.  Uses only workspace memory for staging. */
+ * output device->host, synchronises.  Uses only workspace memory for staging.  When host_s_rec / host_p_rec are
+ * requested the adjoint variables inside the ctx are overwritten (pm_get_adjoint then returns PM_ESTATE). */
 int pm_run_fwd_adj_host(pm_ctx *ctx, const float *host_s0, const float *host_p0,
                         const float *host_delta_target, float *host_s_n, float *host_p_n, double *host_J,
-                        float *host_xi0, float *host_pi0, float *host_dJ_ds0);
+                        float *host_xi0, float *host_pi0, float *host_dJ_ds0, float *host_s_rec, float *host_p_rec);
 
 /* ---- instrumentation ---------------------------------------------------------------------------------
  * When enabled, every kernel launch / cuFFT call of the library is bracketed by CUDA events on the

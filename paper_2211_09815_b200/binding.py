@@ -10,7 +10,8 @@ import os
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libpm.so")
+# PM_LIB selects another build of the same library (e.g. the probe build libpm_debug.so of build.py --debug)
+LIB_PATH = os.environ.get("PM_LIB") or os.path.join(_HERE, "libpm.so")
 
 if not os.path.exists(LIB_PATH):
     # a fresh checkout on a box with nvcc: compile once (under a lock, ranks may import concurrently); never a fallback
@@ -64,7 +65,7 @@ _SIGS = {
     "pm_step_adj": (_int, [_vp, _int]),
     "pm_get_adjoint": (_int, [_vp, _vp, _vp, _vp]),
     "pm_run_fwd_adj": (_int, [_vp] + [_vp] * 5 + [C.POINTER(_dbl)] + [_vp] * 5),
-    "pm_run_fwd_adj_host": (_int, [_vp] + [_vp] * 5 + [C.POINTER(_dbl)] + [_vp] * 3),
+    "pm_run_fwd_adj_host": (_int, [_vp] + [_vp] * 5 + [C.POINTER(_dbl)] + [_vp] * 5),
     "pm_timing_enable": (_int, [_vp, _int]),
     "pm_timing_reset": (_int, [_vp]),
     "pm_timing_read": (_int, [_vp, _int, C.POINTER(C.c_char_p), C.POINTER(_dbl), C.POINTER(_i64), C.POINTER(_dbl)]),
@@ -285,7 +286,7 @@ class PM:
         J = _dbl(0.0)
         g = lambda k: _hptr(out.get(k), k)
         self._call(_lib.pm_run_fwd_adj_host, _hptr(s0, "s0"), _hptr(p0, "p0"), _hptr(delta_target, "delta_target"),
-                   g("s_n"), g("p_n"), C.byref(J), g("xi0"), g("pi0"), g("dJ_ds0"))
+                   g("s_n"), g("p_n"), C.byref(J), g("xi0"), g("pi0"), g("dJ_ds0"), g("s_rec"), g("p_rec"))
         return J.value
 
     # ---- instrumentation ----

@@ -33,6 +33,28 @@ bool pdl_enabled()
     return v == 1;
 }
 
+bool smem_attr_needed(pm_ctx *c, unsigned long long *mask)
+{
+    if (c->device < 0 || c->device >= 64) return true;
+    const unsigned long long bit = 1ull << c->device;
+    if (*mask & bit) return false;
+    *mask |= bit;
+    return true;
+}
+
+// after a stream synchronisation: did a work-queue watchdog fire (pm_cic.cu wq_pop)?  It cannot unless an invariant of
+// the queue is broken; then the results are incomplete and the call reports it instead of hanging the GPU.
+int check_watchdog(pm_ctx *c)
+{
+    int h[16];
+    PM_CUDA(c, cudaMemcpy(h, c->sched, sizeof h, cudaMemcpyDeviceToHost));
+    if (h[8] || h[10]) {
+        cudaMemset(c->sched, 0, 64 * sizeof(int));
+        return fail(c, PM_ECUDA, "work-queue watchdog", "a CIC kernel gave up waiting on its work queue; results are incomplete");
+    }
+    return PM_OK;
+}
+
 Timer::Timer(pm_ctx *ctx, int cls, double bytes) : c(ctx), idx(-1)
 {
     if (cls == TC_FFT_R2C || cls == TC_FFT_C2R) c->n_fft++; else c->n_own++;
@@ -126,6 +148,15 @@ struct Carve {
     }
 };
 
+// global integer accumulators for split scatter tiles (8 KB each): one per 32 tiles, at least 1024 (or every tile)
+static int scatter_pool_slots(const Geometry &g)
+{
+    int n = g.ntiles / 32;
+    if (n < 1024) n = 1024;
+    if (n > g.ntiles) n = g.ntiles;
+    return n;
+}
+
 static size_t fft_work_reserve(const Geometry &g) { return 2 * sizeof(float) * (size_t)g.mesh_stride + (32u << 20); }
 
 static size_t carve_workspace(pm_ctx *c, const Geometry &g, void *base)
@@ -137,10 +168,14 @@ static size_t carve_workspace(pm_ctx *c, const Geometry &g, void *base)
     int *cursor = w.take<int>((size_t)g.nkeys + 1);
     int *hist = w.take<int>((size_t)g.nkeys + 1);
     int *sched = w.take<int>(64);
-    const long long wq_ints = 16 + 8 * ((long long)g.np / GCHUNK + g.ntiles + 64);
+    // work queues (one per stream), 8 ints per item.  Worst case of items: the scatter queues the chunks (2048 records)
+    // of tiles whose record runs hold up to 8 np records in all (a particle is visited by its own tile and by up to 7
+    // high-side neighbours), the gather np / 1024 chunks: np / 256 items cover both.
+    const long long wq_ints = 16 + 8 * ((long long)g.np / 256 + g.ntiles + 64);
     int *wq = w.take<int>((size_t)(2 * wq_ints));
-    int *spool_ctl = w.take<int>(16 + 1024);
-    unsigned *spool = w.take<unsigned>((size_t)1024 * TX * TY * TZ);
+    const int spool_n = scatter_pool_slots(g);
+    int *spool_ctl = w.take<int>(16 + (size_t)spool_n);
+    unsigned *spool = w.take<unsigned>((size_t)spool_n * TX * TY * TZ);
     unsigned long long *scan_agg = w.take<unsigned long long>((size_t)(g.nkeys + 1) / 4096 + 2);
     long long *x = w.take<long long>((size_t)g.np * 3);
     long long *p = w.take<long long>((size_t)g.np * 3);
@@ -156,7 +191,7 @@ static size_t carve_workspace(pm_ctx *c, const Geometry &g, void *base)
     void *fftw = w.take<char>(fft_work_reserve(g));
     if (c) {
         for (int k = 0; k < 7; k++) c->mesh[k] = m + (size_t)k * g.mesh_stride;
-        c->rec = rec; c->offsets = offsets; c->cursor = cursor; c->hist = hist; c->sched = sched; c->wq = wq; c->wq_ints = wq_ints; c->spool_ctl = spool_ctl; c->spool = spool; c->scan_agg = scan_agg;
+        c->rec = rec; c->offsets = offsets; c->cursor = cursor; c->hist = hist; c->sched = sched; c->wq = wq; c->wq_ints = wq_ints; c->spool_ctl = spool_ctl; c->spool = spool; c->spool_n = spool_n; c->scan_agg = scan_agg;
         c->x = x; c->p = p; c->acc = acc; c->xi = xi; c->pi = pi; c->alpha = alpha;
         c->scal = scal; c->ktab = ktab; c->ktabn = tabn;
         c->fft_tab = ffttab;
@@ -250,6 +285,11 @@ static int upload_ktab(pm_ctx *c)
     return PM_OK;
 }
 
+#ifdef PM_DEBUG
+int dbg_prec_init(pm_ctx *c);      // pm_debug_prec.cu
+void dbg_prec_destroy(pm_ctx *c);
+#endif
+
 }  // namespace pm
 
 using namespace pm;
@@ -328,30 +368,37 @@ int pm_init(pm_ctx **out, const pm_params *params, void *dev_workspace, size_t b
     c->scan_epoch = 0;
     c->wq_epoch = 0;
     if (rc == PM_OK && cudaMemsetAsync(c->wq, 0, sizeof(int) * (size_t)(2 * c->wq_ints), c->stream) != cudaSuccess) rc = fail(c, PM_ECUDA, "pm_init", "clearing the gather work queue");
-    if (rc == PM_OK && (cudaMemsetAsync(c->spool_ctl, 0, sizeof(int) * (16 + 1024), c->stream) != cudaSuccess ||
-                        cudaMemsetAsync(c->spool, 0, sizeof(unsigned) * (size_t)1024 * TX * TY * TZ, c->stream) != cudaSuccess))
+    if (rc == PM_OK && (cudaMemsetAsync(c->spool_ctl, 0, sizeof(int) * (16 + (size_t)c->spool_n), c->stream) != cudaSuccess ||
+                        cudaMemsetAsync(c->spool, 0, sizeof(unsigned) * (size_t)c->spool_n * TX * TY * TZ, c->stream) != cudaSuccess))
         rc = fail(c, PM_ECUDA, "pm_init", "clearing the scatter accumulator pool");
     c->overlap_ok = false;
+    c->stream2 = nullptr;
+    c->ev_fork = c->ev_xforce = c->ev_join = nullptr;
     {
         const char *e = getenv("PM_OVERLAP");
         if (!(e && atoi(e) == 0) && cudaStreamCreateWithFlags(&c->stream2, cudaStreamNonBlocking) == cudaSuccess) {
             bool ok = cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) == cudaSuccess;
             ok = ok && cudaEventCreateWithFlags(&c->ev_xforce, cudaEventDisableTiming) == cudaSuccess;
             ok = ok && cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming) == cudaSuccess;
-            c->overlap_ok = ok;
+            c->overlap_ok = ok;  // whatever was created is destroyed by pm_destroy either way
+        } else {
+            c->stream2 = nullptr;
         }
         (void)cudaGetLastError();
     }
     {
-        int dev = 0;
+        c->device = 0;
         c->num_sms = 148;
-        if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, dev);
+        if (cudaGetDevice(&c->device) == cudaSuccess) cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, c->device);
     }
     if (rc == PM_OK && cudaMemsetAsync(c->sched, 0, 64 * sizeof(int), c->stream) != cudaSuccess) rc = fail(c, PM_ECUDA, "pm_init", "clearing the tile scheduler");
     if (rc == PM_OK && (cudaMemsetAsync(c->scan_agg, 0, sizeof(unsigned long long) * ((size_t)(g.nkeys + 1) / 4096 + 2), c->stream) != cudaSuccess ||
                         cudaMemsetAsync(c->hist, 0, sizeof(int) * ((size_t)g.nkeys + 1), c->stream) != cudaSuccess ||
                         cudaStreamSynchronize(c->stream) != cudaSuccess))
         rc = fail(c, PM_ECUDA, "pm_init", "clearing the key histogram");
+#ifdef PM_DEBUG
+    if (rc == PM_OK) rc = dbg_prec_init(c);
+#endif
     if (rc != PM_OK) {
         g_err_noctx = c->err;
         pm_destroy(c);
@@ -364,18 +411,21 @@ int pm_init(pm_ctx **out, const pm_params *params, void *dev_workspace, size_t b
 int pm_destroy(pm_ctx *c)
 {
     if (!c) return PM_OK;
+#ifdef PM_DEBUG
+    dbg_prec_destroy(c);
+#endif
     if (c->plans_ok) {
         cufftDestroy(c->plan_r2c1);
         cufftDestroy(c->plan_c2r1);
     }
     for (auto &r : c->trecs) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
     for (auto e : c->event_pool) cudaEventDestroy(e);
-    if (c->overlap_ok) {
-        cudaEventDestroy(c->ev_fork);
-        cudaEventDestroy(c->ev_xforce);
-        cudaEventDestroy(c->ev_join);
-        cudaStreamDestroy(c->stream2);
-    }
+    if (c->stream2) cudaStreamSynchronize(c->stream2);
+    if (c->ev_fork) cudaEventDestroy(c->ev_fork);
+    if (c->ev_xforce) cudaEventDestroy(c->ev_xforce);
+    if (c->ev_join) cudaEventDestroy(c->ev_join);
+    if (c->stream2) cudaStreamDestroy(c->stream2);
+    (void)cudaGetLastError();
     delete c;
     return PM_OK;
 }

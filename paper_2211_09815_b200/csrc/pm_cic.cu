@@ -8,13 +8,13 @@
 //
 // Input: the records sorted by (tile, class) of pm_bin.cu; a tile is TX x TY x TZ cells.
 //
-// Both kernels are PERSISTENT and WARP-SPECIALISED: a few CTAs per SM, each with one producer warp and
-// NCW consumer warps that talk through a ring of NST shared-memory stages guarded by full / empty
-// mbarriers.  The producer draws the next non-empty tile from a global counter (dense tiles do not stall
-// a static schedule), looks up its record runs, and starts the asynchronous copies of everything the
-// tile needs -- records by 1-D bulk copies, mesh halos by one TMA tensor load per mesh (tiles whose halo
-// wraps around the periodic edge: one bulk copy per halo row) -- all signalled on the stage's full
-// barrier, so the copies of tile n + 1 fly while the consumers work on tile n.
+// Both kernels are PERSISTENT: a few CTAs per SM draw tiles from a global counter (dense tiles do not stall a
+// static schedule).  The scatter is WARP-SPECIALISED: one producer warp looks up the record runs of the next
+// tiles and stages their records in a ring of NST shared-memory stages guarded by full / empty mbarriers (1-D
+// bulk copies + 16-byte cp.async), NCW consumer warps accumulate.  The gather is a two-stage cp.async pipeline in
+// which all 256 threads first start the 16-byte copies of the NEXT tile's halo rows and then interpolate for the
+// particles of the current one (TMA tensor loads of these narrow 144-byte rows were measured slower and removed;
+// TMA is kept for the scatter's tile stores).
 //
 // scatter -- OUTPUT-STATIONARY: the CTA owns the mesh points of the tile, takes the particles of the
 //   tile itself plus the last-cell-layer classes of its (up to 7) low-side neighbour tiles, accumulates in
@@ -31,6 +31,12 @@
 
 #include "pm_pos.cuh"
 
+#ifdef PM_DEBUG
+#define PM_DBG(x) (x)
+#else
+#define PM_DBG(x) 0
+#endif
+
 namespace pm {
 
 struct CicGeom {
@@ -40,17 +46,18 @@ struct CicGeom {
     long long ms;  // floats per mesh (component stride)
     int use_tma;   // scatter: tensor map valid for this mesh; gather: base and strides are 16-byte aligned (async row copies)
     int c0;        // first component (4th tensor-map coordinate)
-    int dbg;       // debug bits (PM_DEBUG_CIC): 1 = gather skips the particle loop, 2 = gather skips the halo copies
-    int kshift;    // debug: coarsen the scatter's fixed-point scale by this many bits (0 in production)
+    int dbg;       // probe build (-DPM_DEBUG) only: 1 = gather skips the particle loop, 2 = skips the halo copies, 8 = clock stamps
+    int kshift;    // probe build only: coarsen the scatter's fixed-point scale by this many bits; both are 0 and unread in libpm.so
     int ntiles;
     double mean;   // unit-mass scatter only: constant subtracted from every mesh point IN INTEGER, before the
                    // int -> fp32 conversion (0 = plain density; nbar on the force path, whose k = 0 mode is zeroed
                    // anyway, so that fp32 rounding is relative to the fluctuation rho - nbar, not to rho)
     long long *dbgbuf;  // debug timeline (PM_DEBUG_CIC & 8): clock64 stamps of CTA 0
     int *spool_ctl;     // scatter pool: [0] next free accumulator, [16 + p] chunks of accumulator p that have arrived
-    unsigned *spool;    // scatter pool: SPOOL_N accumulators of TILE_PTS uint32, all zero between uses
-    int *wq;       // gather overflow queue (pm_internal.cuh); items tagged with wq_epoch
+    unsigned *spool;    // scatter pool: spool_n accumulators of TILE_PTS uint32, all zero between uses
+    int *wq;       // work queue of this stream (wq_reserve / wq_pop below); items tagged with wq_epoch
     int wq_cap;    // items the queue holds
+    int spool_n;   // accumulators in the scatter pool
     unsigned wq_epoch;
     int sh1, sh2;  // log2 of nt[1], nt[2] when they are powers of two (tile index -> coordinates without a division), else -1
     int *sched;    // [0] tile counter, [1] finished CTAs; both zero between launches (the last CTA resets them)
@@ -65,7 +72,6 @@ constexpr int NCW = 8;                                    // consumer warps
 constexpr int NCT = NCW * 32;                             // consumer threads
 constexpr int NTHREADS = NCT + 32;                        // + one producer warp
 constexpr int SCHUNK = 2048;                               // scatter: records per chunk of a heavy tile
-constexpr int SPOOL_N = 1024;                              // scatter: global accumulators for heavy tiles (8 KB each)
 constexpr int RCAP = 512;                                 // records staged in shared memory per tile (the rest are read from global)
 
 // ---- PTX wrappers: mbarrier + TMA (sm_90+/sm_100a) ----------------------------------------------------
@@ -116,13 +122,6 @@ __device__ __forceinline__ bool mbar_test(unsigned long long *bar, unsigned phas
                  : "r"(smem_u32(bar)), "r"(phase)
                  : "memory");
     return ok != 0;
-}
-__device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *m, unsigned long long *bar, int z, int y, int x, int c)
-{
-    asm volatile(
-        "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];"
-        ::"r"(smem_u32(dst)), "l"((unsigned long long)m), "r"(smem_u32(bar)), "r"(z), "r"(y), "r"(x), "r"(c)
-        : "memory");
 }
 __device__ __forceinline__ void bulk_load(void *dst, const void *src, unsigned bytes, unsigned long long *bar)
 {
@@ -199,16 +198,21 @@ static CicGeom make_cic_geom(pm_ctx *c, const float *mesh, int C, int zs, long l
     r.ms = ms;
     r.use_tma = 0;
     r.c0 = 0;
-    // debug knobs, read once per process
+    r.kshift = 0;
+    r.dbg = 0;
+#ifdef PM_DEBUG
+    // probe build only (python -m paper_2211_09815_b200.build --debug -> libpm_debug.so): knobs that change or skip work
     static const int env_kshift = [] { const char *e = getenv("PM_DEBUG_KSHIFT"); return e ? atoi(e) : 0; }();
     static const int env_dbg = [] { const char *e = getenv("PM_DEBUG_CIC"); return e ? atoi(e) : 0; }();
     r.kshift = env_kshift;
+    r.dbg = env_dbg;
+#endif
     r.mean = 0.0;
     r.ntiles = g.ntiles;
-    r.dbg = env_dbg;
     r.sched = c->sched;
     r.wq = c->wq;
-    r.wq_cap = (int)((c->wq_ints - 16) / (store ? 8 : 4));  // scatter items are 8 ints, gather items 4
+    r.wq_cap = (int)((c->wq_ints - 16) / 8);  // WQ_ITEM ints per item
+    r.spool_n = c->spool_n;
     r.spool_ctl = c->spool_ctl;
     r.spool = c->spool;
     r.wq_epoch = ++c->wq_epoch ? c->wq_epoch : ++c->wq_epoch;  // never 0 (the cleared buffer's tag)
@@ -292,6 +296,80 @@ __device__ __forceinline__ void sched_finish(int *sched, int *wq = nullptr, int 
         }
         if (spool_ctl) spool_ctl[0] = 0;
         __threadfence();
+    }
+}
+
+// ---- global work queue for the chunks of heavy tiles (one queue per stream) ----------
+// wq[0] = head, wq[1] = tail, wq[2] = tiles published so far; items of WQ_ITEM ints from wq + 16:
+// {tile, lo, hi, pool, -, -, -, tag}.  ONE layout for the scatter and the gather kernels, so the tag word of an item only
+// ever holds tags (the epoch of the launch that wrote it), never a payload that could be mistaken for one.
+// Pusher (the thread that drew a heavy tile): reserve k items with one fetch-and-add on the tail, write the payloads,
+// fence, write the tags.  The tail is NEVER taken back: when the reservation does not fit, the part below the capacity
+// is published as no-op items (tile = -2) and the tile stays whole, so every reserved index below the capacity is
+// eventually tagged.  Popper (a CTA whose tile counter is exhausted): fetch-and-add on the head; an index below the tail
+// waits for its tag (its pusher is a resident CTA between two consecutive stores); an index at or beyond the tail waits
+// until an item is pushed there or every tile has been published (wq[2] == ntiles: no push can follow), then the CTA is
+// finished for good.  Every wait is on a CTA that has already drawn a tile, i.e. that is resident and itself waits on
+// nobody, which is the forward-progress argument; a watchdog bounds the spins anyway and raises sched[8].
+constexpr int WQ_ITEM = 8;
+constexpr long long WQ_SPIN_CYCLES = 1ll << 33;  // ~4 s at 2 GHz: only a broken invariant gets here
+
+__device__ __forceinline__ int wq_vload(const int *p) { return *reinterpret_cast<const volatile int *>(p); }
+__device__ __forceinline__ void wq_watchdog_fire(const CicGeom &g) { atomicExch(&g.sched[8], 1); }
+
+__device__ __forceinline__ void wq_write(const CicGeom &g, int idx, int tile, int lo, int hi, int pool)
+{
+    int *it = g.wq + 16 + WQ_ITEM * idx;
+    it[0] = tile;
+    it[1] = lo;
+    it[2] = hi;
+    it[3] = pool;
+}
+__device__ __forceinline__ void wq_tag(const CicGeom &g, int idx)
+{
+    *reinterpret_cast<volatile unsigned *>(g.wq + 16 + WQ_ITEM * idx + 7) = g.wq_epoch;
+}
+// one thread: reserves k items; returns their base, or -1 when they do not fit (no-op items published instead)
+__device__ __forceinline__ int wq_reserve(const CicGeom &g, int k)
+{
+    const int base = atomicAdd(&g.wq[1], k);
+    if (base + k <= g.wq_cap) return base;
+    const int end = min(base + k, g.wq_cap);
+    for (int i = base; i < end; i++) wq_write(g, i, -2, 0, 0, -1);
+    __threadfence();
+    for (int i = base; i < end; i++) wq_tag(g, i);
+    __threadfence();
+    return -1;
+}
+// one thread: next item of the queue; false = no more work for this CTA (it must then stay finished)
+__device__ __forceinline__ bool wq_pop(const CicGeom &g, int &tile, int &lo, int &hi, int &pool)
+{
+    for (;;) {
+        const int idx = atomicAdd(&g.wq[0], 1);
+        const long long t_start = clock64();
+        for (;;) {
+            int t = wq_vload(&g.wq[1]);
+            if (idx < t) break;
+            if (wq_vload(&g.wq[2]) == g.ntiles) {
+                __threadfence();
+                t = wq_vload(&g.wq[1]);
+                if (idx >= t) return false;
+                break;
+            }
+            if (clock64() - t_start > WQ_SPIN_CYCLES) { wq_watchdog_fire(g); return false; }
+        }
+        if (idx >= g.wq_cap) return false;  // reservations beyond the capacity hold no items (their tiles stayed whole)
+        const int *it = g.wq + 16 + WQ_ITEM * idx;
+        while ((unsigned)wq_vload(it + 7) != g.wq_epoch) {
+            if (clock64() - t_start > WQ_SPIN_CYCLES) { wq_watchdog_fire(g); return false; }
+        }
+        __threadfence();
+        tile = wq_vload(it);
+        lo = wq_vload(it + 1);
+        hi = wq_vload(it + 2);
+        pool = wq_vload(it + 3);
+        if (tile >= 0) return true;
+        // a no-op item: take the next one
     }
 }
 
@@ -511,29 +589,19 @@ __global__ void __launch_bounds__(NTHREADS) scatter_kernel(const __grid_constant
                 int lo = 0, hi = -1, pool = -1;
                 if (!HAS_VAL && C == 1 && total > SCHUNK + SCHUNK / 2) {
                     const int k = (total + SCHUNK - 1) / SCHUNK;
-                    int base = 0;
+                    int base = -1;
                     if (lane == 0) {
                         pool = atomicAdd(&g.spool_ctl[0], 1);
-                        if (pool < SPOOL_N) {
-                            base = atomicAdd(&g.wq[1], k - 1);
-                            if (base + k - 1 > g.wq_cap) { atomicSub(&g.wq[1], k - 1); pool = -1; }
-                        } else {
-                            pool = -1;
-                        }
+                        if (pool < g.spool_n) base = wq_reserve(g, k - 1);
+                        if (base < 0) pool = -1;  // no accumulator or no room in the queue: the tile stays whole
                     }
                     pool = __shfl_sync(0xffffffffu, pool, 0);
                     base = __shfl_sync(0xffffffffu, base, 0);
                     if (pool >= 0) {
-                        for (int i = lane; i < k - 1; i += 32) {
-                            int *it = g.wq + 16 + 8 * (base + i);
-                            it[0] = tile;
-                            it[1] = SCHUNK * (i + 1);
-                            it[2] = min(total, SCHUNK * (i + 2));
-                            it[3] = pool;
-                        }
+                        for (int i = lane; i < k - 1; i += 32) wq_write(g, base + i, tile, SCHUNK * (i + 1), min(total, SCHUNK * (i + 2)), pool);
                         __threadfence();
                         __syncwarp();
-                        for (int i = lane; i < k - 1; i += 32) *reinterpret_cast<volatile unsigned *>(g.wq + 16 + 8 * (base + i) + 4) = g.wq_epoch;
+                        for (int i = lane; i < k - 1; i += 32) wq_tag(g, base + i);
                         __threadfence();
                         hi = SCHUNK;
                     }
@@ -546,25 +614,7 @@ __global__ void __launch_bounds__(NTHREADS) scatter_kernel(const __grid_constant
             // the tile counter is exhausted: chunks from the queue (fetch-and-add head; see the gather kernel), then finish
             int it_tile = -1, it_lo = 0, it_hi = 0, it_pool = -1;
             if (lane == 0 && !draw_done) {
-                const int idx = atomicAdd(&g.wq[0], 1);
-                for (;;) {
-                    int t = *reinterpret_cast<volatile int *>(&g.wq[1]);
-                    if (idx >= t && *reinterpret_cast<volatile int *>(&g.wq[2]) == g.ntiles) {
-                        __threadfence();
-                        t = *reinterpret_cast<volatile int *>(&g.wq[1]);
-                        if (idx >= t) break;
-                    }
-                    if (idx < t) {
-                        int *it = g.wq + 16 + 8 * idx;
-                        while (*reinterpret_cast<volatile unsigned *>(it + 4) != g.wq_epoch) {}
-                        __threadfence();
-                        it_tile = *reinterpret_cast<volatile int *>(it);
-                        it_lo = *reinterpret_cast<volatile int *>(it + 1);
-                        it_hi = *reinterpret_cast<volatile int *>(it + 2);
-                        it_pool = *reinterpret_cast<volatile int *>(it + 3);
-                        break;
-                    }
-                }
+                if (!wq_pop(g, it_tile, it_lo, it_hi, it_pool)) it_tile = -1;
             }
             it_tile = __shfl_sync(0xffffffffu, it_tile, 0);
             if (it_tile < 0) {
@@ -611,7 +661,7 @@ __global__ void __launch_bounds__(NTHREADS) scatter_kernel(const __grid_constant
     for (int c = 0; c < C; c++) pva[c] = pvb[c] = 0.f;
     for (int n = 0;; n++) {
         const int s = n % NST, b = n & 1;
-#define PM_SSTAMP(k) do { if ((g.dbg & 8) && blockIdx.x == 0 && n < 40 && (tid == 0 || tid == NCT - 1)) g.dbgbuf[((tid ? 1 : 0) * 40 + n) * 12 + (k)] = clock64(); } while (0)
+#define PM_SSTAMP(k) do { if (PM_DBG(g.dbg & 8) && blockIdx.x == 0 && n < 40 && (tid == 0 || tid == NCT - 1)) g.dbgbuf[((tid ? 1 : 0) * 40 + n) * 12 + (k)] = clock64(); } while (0)
         PM_SSTAMP(0);
         mbar_wait(&full[s], (n / NST) & 1);
         PM_SSTAMP(1);
@@ -643,7 +693,7 @@ __global__ void __launch_bounds__(NTHREADS) scatter_kernel(const __grid_constant
             // overflow: sum of weights at a point <= total, and each of the <= total deposits rounds by <= 0.5.
             const float room = fmaxf(4294967296.f * 0.99999f - (float)total, 1.f);
             scale = room / fmaxf((float)total, 1.f);
-            if (g.kshift) scale = ldexpf(scale, -g.kshift);
+            if (PM_DBG(g.kshift)) scale = ldexpf(scale, -g.kshift);
             for (int i = lo + tid; i < hi; i += NCT) {
                 const uint4 q = fetch(i);
                 if (i < n0) {
@@ -714,7 +764,7 @@ __global__ void __launch_bounds__(NTHREADS) scatter_kernel(const __grid_constant
                 }
                 const float M = consumer_max((float)um * 1.0000002f, redf);  // (float) may round down: one ulp up
                 const float bound = (M + 0.5f * (float)total + 1.f) / sA * 1.001f;
-                const int k = min(30 - exp_above(fmaxf(bound, 1e-37f)), 96) - g.kshift;
+                const int k = min(30 - exp_above(fmaxf(bound, 1e-37f)), 96) - PM_DBG(g.kshift);
                 scale = __uint_as_float((unsigned)(127 + k) << 23);
                 auto pass_b = [&](int i, uint4 q, const float v[C]) {
                     float vs[C];
@@ -777,7 +827,7 @@ __global__ void __launch_bounds__(NTHREADS) scatter_kernel(const __grid_constant
         }
 
         PM_SSTAMP(2);
-        if ((g.dbg & 8) && blockIdx.x == 0 && n < 40 && tid == 0) g.dbgbuf[n * 12 + 11] = sl.total;
+        if (PM_DBG(g.dbg & 8) && blockIdx.x == 0 && n < 40 && tid == 0) g.dbgbuf[n * 12 + 11] = sl.total;
         if (tid == 0) tma_store_wait_read();  // the previous tile's store has read the other buffer out
         PM_SSTAMP(3);
         consumer_sync();                      // all deposits of this tile are in; the other buffer is free
@@ -1011,9 +1061,7 @@ __global__ void __launch_bounds__(GT) gather_kernel(CicGeom g, const uint4 *__re
     };
     // Publishing a drawn tile.  A tile with more than GCHUNK particles is split: the first chunk is published, the others
     // go to a global queue from which any CTA takes them once the tile counter is exhausted (a dense clump would
-    // otherwise keep one CTA busy long after all others have finished).  A pusher reserves its items with one atomic on
-    // the tail, writes them and tags them with this launch's epoch; a popper advances the head by compare-and-swap, so
-    // the head never passes the tail and an item pushed late is still found by whoever is alive (at least its pusher).
+    // otherwise keep one CTA busy long after all others have finished); protocol: see wq_reserve / wq_pop above.
     bool draw_done = false;  // drawing thread only
     auto publish_range = [&](GatherSlot &dst, int tile, int beg, int end) {
         dst.tile = tile;
@@ -1029,20 +1077,13 @@ __global__ void __launch_bounds__(GT) gather_kernel(CicGeom g, const uint4 *__re
             int end = d.end;
             if (end - d.beg > GCHUNK) {
                 const int k = (end - d.beg + GCHUNK - 1) / GCHUNK - 1;
-                const int base = atomicAdd(&g.wq[1], k);
-                if (base + k <= g.wq_cap) {
-                    for (int i = 0; i < k; i++) {
-                        int *it = g.wq + 16 + 4 * (base + i);
-                        it[0] = d.tile;
-                        it[1] = d.beg + GCHUNK * (i + 1);
-                        it[2] = min(d.end, d.beg + GCHUNK * (i + 2));
-                    }
+                const int base = wq_reserve(g, k);
+                if (base >= 0) {
+                    for (int i = 0; i < k; i++) wq_write(g, base + i, d.tile, d.beg + GCHUNK * (i + 1), min(d.end, d.beg + GCHUNK * (i + 2)), -1);
                     __threadfence();
-                    for (int i = 0; i < k; i++) *reinterpret_cast<volatile unsigned *>(g.wq + 16 + 4 * (base + i) + 3) = g.wq_epoch;
+                    for (int i = 0; i < k; i++) wq_tag(g, base + i);
                     __threadfence();  // the tail update and the items are visible before this tile counts as published
                     end = d.beg + GCHUNK;
-                } else {
-                    atomicSub(&g.wq[1], k);  // cannot happen with the sized queue; keep the tile whole
                 }
             }
             publish_range(dst, d.tile, d.beg, end);
@@ -1050,25 +1091,14 @@ __global__ void __launch_bounds__(GT) gather_kernel(CicGeom g, const uint4 *__re
             return;
         }
         // the tile counter is exhausted: take a chunk from the queue, or finish (and stay finished: the CTA stops at the
-        // first slot marked -1, so nothing may be taken from the queue after that).  The head is advanced by a plain
-        // fetch-and-add (a compare-and-swap loop collapses when hundreds of CTAs pop at once); an index beyond the tail
-        // waits until either an item is pushed there or every tile has been published (wq[2] == ntiles: no more pushes).
+        // first slot marked -1, so nothing may be taken from the queue after that)
         if (draw_done) { dst.tile = -1; return; }
-        const int idx = atomicAdd(&g.wq[0], 1);
-        for (;;) {
-            int t = *reinterpret_cast<volatile int *>(&g.wq[1]);
-            if (idx >= t && *reinterpret_cast<volatile int *>(&g.wq[2]) == g.ntiles) {
-                __threadfence();
-                t = *reinterpret_cast<volatile int *>(&g.wq[1]);
-                if (idx >= t) { draw_done = true; dst.tile = -1; return; }
-            }
-            if (idx < t) {
-                int *it = g.wq + 16 + 4 * idx;
-                while (*reinterpret_cast<volatile unsigned *>(it + 3) != g.wq_epoch) {}
-                __threadfence();
-                publish_range(dst, *reinterpret_cast<volatile int *>(it), *reinterpret_cast<volatile int *>(it + 1), *reinterpret_cast<volatile int *>(it + 2));
-                return;
-            }
+        int qt, qlo, qhi, qpool;
+        if (wq_pop(g, qt, qlo, qhi, qpool)) {
+            publish_range(dst, qt, qlo, qhi);
+        } else {
+            draw_done = true;
+            dst.tile = -1;
         }
     };
     if (tid == DRAWER) {
@@ -1100,14 +1130,14 @@ __global__ void __launch_bounds__(GT) gather_kernel(CicGeom g, const uint4 *__re
     auto body = [&](const int n, DrawSet &Spub, DrawSet &Sfill, int &a_use, int &a_new) -> bool {
         const GatherSlot cur = slot[n & 7];
         if (cur.tile < 0) return false;
-#define PM_STAMP(k) do { if ((g.dbg & 8) && blockIdx.x == 0 && n < 40 && (tid == 0 || tid == GT - 1)) g.dbgbuf[((tid ? 1 : 0) * 40 + n) * 12 + (k)] = clock64(); } while (0)
+#define PM_STAMP(k) do { if (PM_DBG(g.dbg & 8) && blockIdx.x == 0 && n < 40 && (tid == 0 || tid == GT - 1)) g.dbgbuf[((tid ? 1 : 0) * 40 + n) * 12 + (k)] = clock64(); } while (0)
         PM_STAMP(0);
-        if ((g.dbg & 8) && blockIdx.x == 0 && n < 40 && tid == 0) g.dbgbuf[n * 12 + 11] = cur.end - cur.beg;
+        if (PM_DBG(g.dbg & 8) && blockIdx.x == 0 && n < 40 && tid == 0) g.dbgbuf[n * 12 + 11] = cur.end - cur.beg;
         // the halo of the tile GST - 1 iterations ahead starts to fly now (its stage was released by the barrier that
         // ended iteration n - 1)
         {
             const GatherSlot far = slot[(n + GST - 1) & 7];
-            if (far.tile >= 0 && far.beg < far.end && !(g.dbg & 2)) halo_issue<C>(g, mesh, far, halo_of((n + GST - 1) % GST));
+            if (far.tile >= 0 && far.beg < far.end && !PM_DBG(g.dbg & 2)) halo_issue<C>(g, mesh, far, halo_of((n + GST - 1) % GST));
         }
         cp_async_commit();
         PM_STAMP(1);
@@ -1117,7 +1147,7 @@ __global__ void __launch_bounds__(GT) gather_kernel(CicGeom g, const uint4 *__re
         if (has_nx) q_nx = rec[nxt.beg + tid];
         // a second round of the current tile (more than GT particles): its record is requested now, its per-particle
         // inputs right after the barrier, so that neither round trip is exposed between the rounds
-        const int cnt = (g.dbg & 1) ? 0 : cur.end - cur.beg;
+        const int cnt = PM_DBG(g.dbg & 1) ? 0 : cur.end - cur.beg;
         uint4 q2 = make_uint4(0, 0, 0, 0);
         if (tid + GT < cnt) q2 = rec[cur.beg + tid + GT];
         cp_async_wait<GST - 1>();  // this thread's copies of the current tile have landed ...
@@ -1209,7 +1239,7 @@ __global__ void __launch_bounds__(GT) gather_kernel(CicGeom g, const uint4 *__re
                     }
                 }
             } else if (MODE == G_VALUE) {
-                if ((g.dbg & 4) && val[0] != 12345.f) continue;
+                if (PM_DBG(g.dbg & 4) && val[0] != 12345.f) continue;
 #pragma unroll
                 for (int c = 0; c < C; c++) out[j * C + c] = val[c];
             } else if (MODE == G_GRAD) {
@@ -1269,11 +1299,8 @@ static cudaError_t allow_smem(K kernel, size_t bytes)
 
 #define PM_CIC_LAUNCH(ctx, name, kernel, threads, smem, ...)                                          \
     do {                                                                                     \
-        static bool attr_done_ = false;                                                      \
-        if (!attr_done_) {                                                                   \
-            PM_CUDA(ctx, allow_smem(kernel, smem));                                          \
-            attr_done_ = true;                                                               \
-        }                                                                                    \
+        static unsigned long long attr_mask_ = 0;                                            \
+        if (smem_attr_needed(ctx, &attr_mask_)) PM_CUDA(ctx, allow_smem(kernel, smem));      \
         PM_CUDA(ctx, launch_pdl(kernel, dim3(persistent_grid(ctx, smem, threads)), dim3(threads), smem, (ctx)->stream, __VA_ARGS__)); \
         PM_LAUNCH_CHECK(ctx, name);                                                          \
     } while (0)

@@ -620,11 +620,12 @@ int fft_own_init(pm_ctx *c)
 
 #define PM_FFT_LAUNCH(ctx, name, kernel, grid, smem, ...)                                  \
     do {                                                                                   \
-        static size_t attr_ = 0;                                                           \
-        if ((smem) > attr_) {                                                              \
-            PM_CUDA(ctx, cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(smem))); \
-            attr_ = (smem);                                                                \
-        }                                                                                  \
+        /* every instantiation is launched with ONE shared-memory size per mesh axis length, the largest it ever needs */ \
+        static unsigned long long attr_mask_ = 0;                                          \
+        static size_t attr_bytes_ = 0;                                                     \
+        if ((smem) > attr_bytes_) { attr_mask_ = 0; attr_bytes_ = (smem); }                \
+        if (smem_attr_needed(ctx, &attr_mask_))                                            \
+            PM_CUDA(ctx, cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)attr_bytes_)); \
         PM_CUDA(ctx, launch_pdl(kernel, dim3(grid), dim3(FFT_T), smem, (ctx)->stream, __VA_ARGS__)); \
         PM_LAUNCH_CHECK(ctx, name);                                                        \
     } while (0)

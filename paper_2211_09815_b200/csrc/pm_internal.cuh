@@ -82,7 +82,7 @@ struct pm_ctx {
     cudaStream_t stream2;        // second stream: the Pi branch of an adjoint step runs beside the force branch
     cudaEvent_t ev_fork, ev_xforce, ev_join;
     bool overlap_ok;             // stream2 and the events exist (and PM_OVERLAP != 0)
-    cufftHandle plan_r2c1, plan_c2r1, plan_r2c3, plan_c2r3;
+    cufftHandle plan_r2c1, plan_c2r1;
     bool plans_ok;
     // workspace carve-up (device pointers)
     float *mesh[7];              // padded in-place R2C layout, contiguous
@@ -92,13 +92,16 @@ struct pm_ctx {
     int *hist;                   // nkeys + 1 key histogram; zero between sorts (the scan clears it)
     unsigned long long *scan_agg;  // scan scratch: per-block totals tagged with the launch epoch
     unsigned int scan_epoch;
-    int *sched;                  // 2 ints: tile counter and finished-CTA count of the persistent CIC kernels (zero between launches)
+    int *sched;                  // per stream (stream2: + 2): [0] tile counter, [1] finished CTAs of the persistent CIC kernels (zero
+                                 // between launches), [8] work-queue watchdog flag (check_watchdog)
     int num_sms;
-    int *wq;                     // overflow work queue of the gathers (chunks of heavy tiles): [0] head, [1] tail, items from [16]
+    int device;                  // CUDA device the ctx was created on
+    int *wq;                     // work queue of the CIC kernels (chunks of heavy tiles): [0] head, [1] tail, [2] tiles published, items from [16]
     long long wq_ints;           // ints per queue (two queues: one per stream)
     unsigned int wq_epoch;       // tag of the items pushed by the current launch
     int *spool_ctl;              // scatter pool control: [0] next accumulator, [16 + p] arrived chunks
-    unsigned *spool;             // scatter pool: 1024 accumulators of one tile (8 KB) each, zero between uses
+    unsigned *spool;             // scatter pool: spool_n accumulators of one tile (8 KB) each, zero between uses
+    int spool_n;
     long long *x;                // [np][3] int64 absolute position (q + s) * 2^XBITS, not wrapped
     long long *p;                // [np][3] int64 momentum * 2^PBITS
     float *acc, *xi, *pi, *alpha;  // [np][3]
@@ -130,6 +133,10 @@ namespace pm {
 
 // record the last error text and return code
 int fail(pm_ctx *c, int code, const char *what, const char *detail);
+// cudaFuncSetAttribute(MaxDynamicSharedMemorySize) is per device: true when (slot, device of ctx) still needs it.
+// slot = a function-local static 64-bit mask at the launch site (devices 0..63; beyond that the attribute is set every time)
+bool smem_attr_needed(pm_ctx *c, unsigned long long *mask);
+int check_watchdog(pm_ctx *c);
 
 #define PM_CUDA(ctx, call)                                                        \
     do {                                                                          \

@@ -216,6 +216,12 @@ def test_config0_forward_adjoint_parity(pmlib, orc):
     assert Jh == out["J"]
     for k in host:
         assert np.array_equal(host[k].numpy(), out[k].cpu().numpy()), k
+    # ... and the exact-reversal property is observable through it too (s_rec, p_rec)
+    host2 = {k: torch.empty((pm.np, 3), dtype=torch.float32).pin_memory() for k in ("dJ_ds0", "s_rec", "p_rec")}
+    pm.run_fwd_adj_host(torch.from_numpy(s0), torch.from_numpy(p0), torch.from_numpy(target), host2)
+    assert np.array_equal(host2["dJ_ds0"].numpy(), out["dJ_ds0"].cpu().numpy())
+    assert np.array_equal(host2["s_rec"].numpy(), s_q.astype(np.float32))
+    assert np.array_equal(host2["p_rec"].numpy(), p_q.astype(np.float32))
     pm.close()
 
 

@@ -1,0 +1,262 @@
+"""GPU parity on the code paths only the larger configs take (run on the B200 box with `-m gpu`):
+
+  * every radix plan of the library's own FFT passes (axes of 16 ... 1024 points) against the ORACLE's force and
+    force VJP on thin meshes the oracle finishes in seconds;
+  * the whole forward + adjoint run of configs[0] with CIC deconvolution switched on (reading R12);
+  * the two-stream adjoint step on a clustered state (heavy tiles: split scatter tiles, gather chunks in the work
+    queues of both streams at once), bit-identical to the one-stream order, under a host-side timeout;
+  * configs[3]/configs[4] sizes (512^3 particles, 1024^3 mesh): pm_scatter against the oracle's scatter on the whole
+    mesh (unit mass) and on sub-boxes (3 components), gathers on sampled particles, for the real configs[4] inputs;
+    own-FFT path against the cuFFT path for pm_force / pm_force_vjp at 1024^3.
+"""
+import numpy as np
+import pytest
+
+from paper_2211_09815_b200 import inputs
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+
+def rel_l2(a, b):
+    a = np.asarray(a, dtype=np.float64)
+    b = np.asarray(b, dtype=np.float64)
+    return float(np.sqrt(np.sum((a - b) ** 2) / max(np.sum(b ** 2), 1e-300)))
+
+
+@pytest.fixture(scope="module")
+def pmlib():
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device (there is no CPU fallback)")
+    from paper_2211_09815_b200 import binding
+    return binding
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda()
+
+
+# One mesh per plan: x / y axes of 16 (radix 16), 32 (8 x 4), 64 (16 x 4), 128 (16 x 8), 256 (16 x 16), 512 (8 x 16 x 4),
+# 1024 (16 x 16 x 4); z axes whose half length Nz/2 runs through 8 ... 512.  Thin in the other directions.
+PLAN_MESHES = [
+    (512, 16, 32), (16, 512, 32), (32, 16, 512), (16, 32, 1024), (32, 32, 32), (1024, 16, 16), (16, 1024, 16),
+    (128, 64, 16), (64, 128, 256), (256, 16, 64), (16, 256, 128),
+]
+
+
+@pytest.mark.parametrize("mesh", PLAN_MESHES)
+@pytest.mark.parametrize("deconv", [0, 1])
+def test_own_fft_plans_against_oracle(pmlib, orc, mesh, deconv, monkeypatch):
+    """pm_force / pm_force_vjp through the own z, y and fused x passes against the oracle (eq. 11 L127-131 and its
+    transpose), rel L2 <= 1e-5, on a mesh with one long axis per radix plan."""
+    if deconv and mesh not in ((512, 16, 32), (16, 32, 1024), (1024, 16, 16)):
+        pytest.skip("deconvolution is covered on three of the plans")
+    monkeypatch.setenv("PM_FFT", "own")   # also above the default own-FFT size limit, if any
+    lattice = tuple(n // 2 for n in mesh)
+    rng = np.random.default_rng(41)
+    pm = pmlib.PM(mesh, lattice, 0.3, [0.5, 1.0], deconvolve=deconv)
+    assert pm.np == int(np.prod(lattice))
+    s = rng.normal(0, 1.2, (pm.np, 3))
+    x = orc.positions(mesh, lattice, s).astype(np.float32)
+    pi = rng.standard_normal((pm.np, 3)).astype(np.float32)
+    acc, alpha = pm.force_vjp(dev(x), dev(pi))
+    own, fft = pm.launch_count()
+    assert fft == 0, "the own FFT path must not call cuFFT"
+    acc_o = orc.force(mesh, 0.3, x, deconv=deconv)
+    alpha_o = orc.force_vjp(mesh, 0.3, x, pi, deconv=deconv)
+    assert rel_l2(acc.cpu().numpy(), acc_o) <= 1e-5
+    assert rel_l2(alpha.cpu().numpy(), alpha_o) <= 1e-5
+    pm.close()
+
+
+def _cfg0_inputs(orc, deconv):
+    cfg = inputs.config(0)
+    s0 = inputs.zeldovich_displacement(cfg["lattice"], cfg["mesh"], seed=1, rms=0.3)
+    ratio = orc.p_over_s(cfg["omega_m"], cfg["a"][0])
+    p0 = (s0.astype(np.float64) * ratio).astype(np.float32)
+    s0t = inputs.zeldovich_displacement(cfg["lattice"], cfg["mesh"], seed=2, rms=0.3)
+    p0t = (s0t.astype(np.float64) * ratio).astype(np.float32)
+    s_nt, _, _ = orc.run_fwd(cfg["mesh"], cfg["lattice"], cfg["omega_m"], cfg["a"], s0t, p0t, deconv=deconv)
+    xt = orc.positions(cfg["mesh"], cfg["lattice"], s_nt)
+    nbar = np.prod(cfg["lattice"]) / np.prod(cfg["mesh"])
+    target = (orc.scatter(cfg["mesh"], xt) / nbar - 1.0).astype(np.float32)
+    return cfg, s0, p0, target
+
+
+@pytest.mark.parametrize("fft", ["own", "cufft"])
+def test_config0_whole_run_with_deconvolution(pmlib, orc, fft, monkeypatch):
+    """SURVEY reading 12: whole-run parity at configs[0] in BOTH deconvolution modes (mode 0 is in test_gpu_parity.py)."""
+    monkeypatch.setenv("PM_FFT", fft)
+    cfg, s0, p0, target = _cfg0_inputs(orc, 1)
+    ref = orc.run_fwd_adj(cfg["mesh"], cfg["lattice"], cfg["omega_m"], cfg["a"], s0, p0, target, deconv=1)
+    pm = pmlib.PM(cfg["mesh"], cfg["lattice"], cfg["omega_m"], cfg["a"], deconvolve=1)
+    out = pm.run_fwd_adj(dev(s0), dev(p0), dev(target))
+    s_n = out["s_n"].cpu().numpy().astype(np.float64)
+    rms = np.sqrt(np.mean(np.sum((s_n - ref["s_n"]) ** 2, axis=1)))
+    assert rms <= 1e-4, f"final positions rms {rms} cell"
+    assert abs(out["J"] - ref["J"]) <= 1e-4 * abs(ref["J"])
+    for k in ("xi0", "pi0", "dJ_ds0"):
+        e = rel_l2(out[k].cpu().numpy(), ref[k])
+        assert e <= 1e-3, f"{k} rel L2 {e}"
+    s_q = np.rint(s0.astype(np.float64) * 2.0 ** 32) / 2.0 ** 32
+    assert np.array_equal(out["s_rec"].cpu().numpy(), s_q.astype(np.float32))
+    pm.close()
+
+
+def _clustered_state(L, N, n_blobs):
+    """displacements that put the lattice particles on the configs[4] blob distribution (generation order)"""
+    mesh = (N, N, N)
+    x = inputs.blob_positions(L ** 3, mesh, seed=3, n_blobs=n_blobs, order="generation").astype(np.float64)
+    q = np.stack(np.meshgrid(*[np.arange(L) * (N // L)] * 3, indexing="ij"), axis=-1).reshape(-1, 3).astype(np.float64)
+    s = x - q
+    s -= N * np.rint(s / N)          # minimum image: |s| <= N/2
+    return mesh, s.astype(np.float32)
+
+
+@pytest.mark.timeout(600, method="thread")
+def test_two_stream_adjoint_on_clustered_state(pmlib, monkeypatch):
+    """Adjoint steps on a state with collapsed clumps: the unit-mass scatter splits heavy tiles through the work queue
+    of the caller's stream while the valued scatter / gathers of the other branch run on stream2 with their own
+    queue.  Must terminate (a broken queue invariant raises PMError through the watchdog instead of hanging) and
+    agree bit for bit with the one-stream order."""
+    L, N = 128, 256
+    mesh, s0 = _clustered_state(L, N, 313)
+    a = inputs.a_schedule(0.5, 3)
+    rng = np.random.default_rng(9)
+    p0 = (0.05 * rng.standard_normal(s0.shape)).astype(np.float32)
+    xi = rng.standard_normal(s0.shape).astype(np.float32)
+    pi = rng.standard_normal(s0.shape).astype(np.float32)
+    outs = {}
+    for mode in ("1", "0"):
+        monkeypatch.setenv("PM_OVERLAP", mode)
+        pm = pmlib.PM(mesh, (L,) * 3, 0.3, a)
+        pm.set_state(dev(s0), dev(p0))
+        for i in range(1, 4):
+            pm.step_fwd(i)
+        pm.set_adjoint(dev(xi), dev(pi))
+        for i in range(3, 0, -1):
+            pm.step_adj(i)
+        torch.cuda.synchronize()
+        outs[mode] = [t.clone() for t in pm.get_adjoint()] + list(pm.get_state())
+        pm.get_objective()   # synchronises and checks the watchdog flags of both streams
+        pm.close()
+    for u, v in zip(outs["1"], outs["0"]):
+        assert torch.equal(u, v)
+    # reversal is exact on this state too
+    s_q = np.rint(s0.astype(np.float64) * 2.0 ** 32) / 2.0 ** 32
+    assert np.array_equal(outs["1"][3].cpu().numpy(), s_q.astype(np.float32))
+
+
+# ---- configs[3] / configs[4] sizes ------------------------------------------------------------------------------------
+BIG_L, BIG_N = 512, 1024
+
+
+def test_config3_force_vjp_own_fft_vs_cufft(pmlib, monkeypatch):
+    """pm_force / pm_force_vjp at 1024^3 on the configs[3] initial state: the library's own transform passes against the
+    cuFFT + stand-alone k-space kernel path (two independent implementations of eq. 11 and its transpose; each is
+    compared with the oracle on the smaller meshes above).  The oracle itself needs ~70 GB of host memory for one
+    force at 1024^3, so at this size the two paths check each other."""
+    cfg = inputs.config(3)
+    s0 = inputs.zeldovich_displacement(cfg["lattice"], cfg["mesh"], seed=1, rms=0.3)
+    q = np.stack(np.meshgrid(*[np.arange(BIG_L, dtype=np.float32) * 2] * 3, indexing="ij"), axis=-1).reshape(-1, 3)
+    x = q + s0
+    rng = np.random.default_rng(29)
+    pi = rng.standard_normal(x.shape).astype(np.float32)
+    res = {}
+    for mode in ("own", "cufft"):
+        monkeypatch.setenv("PM_FFT", mode)
+        pm = pmlib.PM(cfg["mesh"], cfg["lattice"], cfg["omega_m"], [1.0])
+        acc, alpha = pm.force_vjp(torch.from_numpy(x).cuda(), torch.from_numpy(pi).cuda())
+        own, fft = pm.launch_count()
+        assert (fft == 0) == (mode == "own")
+        res[mode] = (acc.cpu().numpy(), alpha.cpu().numpy())
+        pm.close()
+        del acc, alpha
+        torch.cuda.empty_cache()
+    assert rel_l2(res["own"][0], res["cufft"][0]) <= 2e-6
+    assert rel_l2(res["own"][1], res["cufft"][1]) <= 2e-6
+    tot = np.abs(res["own"][0].astype(np.float64).sum(axis=0))
+    assert np.all(tot <= 1e-5 * np.abs(res["own"][0]).sum(axis=0))      # P3 momentum conservation at full size
+
+
+@pytest.fixture(scope="module")
+def big(pmlib):
+    """One ctx of the configs[3] geometry (69.5 GB workspace) shared by the full-size kernel tests."""
+    free, _ = torch.cuda.mem_get_info()
+    need = pmlib.workspace_bytes((BIG_N,) * 3, (BIG_L,) * 3, 0.3, [1.0])
+    if free < need + (24 << 30):
+        pytest.fail(f"configs[3] needs {need / 2**30:.0f} GiB of workspace; {free / 2**30:.0f} GiB free on this device")
+    pm = pmlib.PM((BIG_N,) * 3, (BIG_L,) * 3, 0.3, [1.0])
+    yield pm
+    pm.close()
+
+
+def _subbox_scatter(orc, x, val, lo, size):
+    """The oracle's scatter restricted to the mesh points [lo, lo + size)^3 of the periodic 1024^3 mesh: every particle
+    within one cell of the box is deposited (serially, eq. 10) on a private periodic mesh of 2 x size points, shifted so
+    that the box sits in its middle; deposits from outside the box never reach its interior."""
+    N = BIG_N
+    d = np.mod(x.astype(np.float64) - (np.asarray(lo, dtype=np.float64) - 1.0), N)     # distance above lo - 1
+    sel = np.all(d < size + 2.0, axis=1)
+    m = 2 * size
+    xs = d[sel] - 1.0 + size // 2                                                       # box starts at size // 2
+    out = orc.scatter((m, m, m), xs, None if val is None else val[sel])
+    h = size // 2
+    return out[..., h:h + size, h:h + size, h:h + size], int(sel.sum())
+
+
+@pytest.mark.parametrize("order", ["generation", "random"])
+def test_config4_inputs_full_size_kernel_parity(pmlib, orc, big, order):
+    """The real configs[4] inputs (512^3 particles, 20000 blobs, 1024^3 mesh) in both memory orders: pm_scatter (unit mass)
+    against the oracle's serial scatter on the WHOLE mesh; the 3-component scatter on sub-boxes around the densest
+    cells and at the periodic corner; gathers and weight-gradient gathers on 20000 sampled particles.  This exercises
+    the 64-bit index paths, the 1024-axis tile counts and the work queues / accumulator pool at their real load."""
+    pm = big
+    mesh = (BIG_N,) * 3
+    npart = BIG_L ** 3
+    x = inputs.blob_positions(npart, mesh, seed=3, n_blobs=20000, order=order)
+    xd = torch.from_numpy(x).cuda()
+    rng = np.random.default_rng(23)
+    # --- unit-mass scatter, whole mesh, compared slab by slab (the fp64 mesh of the oracle is 8.6 GB)
+    rho = pm.scatter(xd).cpu().numpy()
+    rho_o = orc.scatter(mesh, x)
+    assert rho_o.max() > 100.0
+    num = den = tot = 0.0
+    for i in range(0, BIG_N, 64):
+        a = rho[i:i + 64].astype(np.float64)
+        b = rho_o[i:i + 64]
+        num += float(np.sum((a - b) ** 2))
+        den += float(np.sum(b ** 2))
+        tot += float(a.sum())
+    assert np.sqrt(num / den) <= 1e-5
+    assert abs(tot - npart) <= 1e-6 * npart
+    # densest cells (for the sub-boxes of the valued scatter) before the big arrays go
+    flat = np.argpartition(rho_o.reshape(-1), -4)[-4:]
+    peaks = [np.unravel_index(int(f), mesh) for f in flat]
+    del rho, rho_o
+    # --- 3-component scatter on sub-boxes of 32^3 points: two around the densest cells, the periodic corner, one random
+    val = (rng.standard_normal((npart, 3)) * np.exp(rng.normal(0, 1.5, (npart, 1)))).astype(np.float32)
+    vd = torch.from_numpy(val).cuda()
+    m3 = pm.scatter(xd, vd)
+    assert abs(float(m3.double().sum()) - float(val.astype(np.float64).sum())) <= 1e-6 * float(np.abs(val).sum())
+    boxes = [tuple((int(p[d]) - 16) % BIG_N for d in range(3)) for p in peaks[:2]] + [(BIG_N - 16,) * 3, (300, 700, 100)]
+    for lo in boxes:
+        ref, nsel = _subbox_scatter(orc, x, val, lo, 32)
+        ix = [torch.from_numpy((np.arange(32) + lo[d]) % BIG_N).cuda() for d in range(3)]
+        got = m3[:, ix[0]][:, :, ix[1]][:, :, :, ix[2]].cpu().numpy()
+        assert nsel > 0 and rel_l2(got, ref) <= 1e-5, f"box {lo}"
+    del m3, vd
+    torch.cuda.empty_cache()
+    # --- gathers on sampled particles
+    gen = torch.Generator(device="cuda").manual_seed(5)
+    fd = torch.randn((3,) + mesh, device="cuda", generator=gen)
+    idx = np.sort(rng.choice(npart, 20000, replace=False))
+    g3 = pm.gather(xd, fd)[torch.from_numpy(idx).cuda()].cpu().numpy()
+    f = fd.cpu().numpy()
+    assert rel_l2(g3, orc.gather(mesh, x[idx], f)) <= 1e-5
+    cot = rng.standard_normal((npart, 3)).astype(np.float32)
+    gg = pm.gather_grad(xd, fd, torch.from_numpy(cot).cuda())[torch.from_numpy(idx).cuda()].cpu().numpy()
+    assert rel_l2(gg, orc.gather_grad(mesh, x[idx], f, cot[idx])) <= 1e-5
+    gs = pm.gather_grad(xd, fd[0].contiguous())[torch.from_numpy(idx).cuda()].cpu().numpy()
+    assert rel_l2(gs, orc.gather_grad(mesh, x[idx], f[0])) <= 1e-5
+    pm.get_objective()   # synchronises and checks the work-queue watchdog
