@@ -43,8 +43,15 @@ typedef struct {
     const double *a;     /* HOST: n_steps + 1 scale factors, strictly increasing, copied by pm_init     */
     int32_t deconvolve;  /* 0 = eq. 11 as printed (L127-131); 1 = also divide by the CIC window^2,
                             prod_d sinc(k_d/2)^-4 (reading R12; not in the paper)            */
-    int32_t flags;       /* reserved, must be 0                                                        */
+    int32_t flags;       /* 0, or PM_FLAG_FP64_TRANSFORMS (below); any other bit is PM_EINVAL           */
 } pm_params;
+
+/* pm_params.flags.  PM_FLAG_FP64_TRANSFORMS: the 3-D transforms and the k-space operators of eq. 11 (L127-131) and of
+   its transpose run in double precision (cuFFT D2Z / Z2D + fp64 kernels) -- the paper's "more precise floating-point
+   numbers" remedy (L371; fp64 rows of Tables 1-2) applied to the one stage whose fp32 rounding limits the
+   gradient (precision A/B).  Every particle and mesh array crossing the ABI stays fp32; the
+   workspace grows by four fp64 meshes plus cuFFT's work area.  Slower; results stay bit-reproducible and reversible. */
+enum { PM_FLAG_FP64_TRANSFORMS = 1 };
 
 enum {
     PM_OK = 0,

@@ -39,6 +39,7 @@ class pm_params(C.Structure):
 
 PM_OK, PM_EINVAL, PM_EWORKSPACE, PM_ECUDA, PM_ECUFFT, PM_ESTATE = 0, -1, -2, -3, -4, -5
 PM_TIMING_MAX_CLASSES = 32
+PM_FLAG_FP64_TRANSFORMS = 1
 
 _vp, _i64, _int, _dbl = C.c_void_p, C.c_int64, C.c_int, C.c_double
 _SIGS = {
@@ -126,8 +127,8 @@ def host_fft_order(n):
     return list(out)
 
 
-def workspace_bytes(mesh, lattice, omega_m, a, deconvolve=0):
-    p, keep = make_params(mesh, lattice, omega_m, a, deconvolve)
+def workspace_bytes(mesh, lattice, omega_m, a, deconvolve=0, flags=0):
+    p, keep = make_params(mesh, lattice, omega_m, a, deconvolve, flags)
     n = C.c_size_t(0)
     rc = _lib.pm_workspace_bytes(C.byref(p), C.byref(n))
     if rc != PM_OK:
@@ -156,7 +157,7 @@ def _hptr(t, name="tensor"):
 class PM:
     """One libpm context.  Method names follow include/pm.h without the pm_ prefix."""
 
-    def __init__(self, mesh, lattice, omega_m, a, deconvolve=0, device="cuda:0", stream=None):
+    def __init__(self, mesh, lattice, omega_m, a, deconvolve=0, device="cuda:0", stream=None, flags=0):
         if not torch.cuda.is_available():
             raise RuntimeError("libpm needs a CUDA device; there is no CPU fallback")
         self.mesh = tuple(int(v) for v in mesh)
@@ -165,7 +166,7 @@ class PM:
         self.ng = self.mesh[0] * self.mesh[1] * self.mesh[2]
         self.n_steps = len(a) - 1
         self.device = torch.device(device)
-        self._params, self._keep = make_params(mesh, lattice, omega_m, a, deconvolve)
+        self._params, self._keep = make_params(mesh, lattice, omega_m, a, deconvolve, flags)
         n = C.c_size_t(0)
         self._h = _vp(None)
         self._check(_lib.pm_workspace_bytes(C.byref(self._params), C.byref(n)), None)

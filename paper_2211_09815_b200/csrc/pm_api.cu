@@ -100,7 +100,7 @@ static int make_geometry(const pm_params *p, Geometry *g, const char **why)
     if (!(p->omega_m > 0.0) || p->omega_m > 1.0) { *why = "omega_m must be in (0, 1]"; return PM_EINVAL; }
     if (p->n_steps < 0) { *why = "n_steps < 0"; return PM_EINVAL; }
     if (p->n_steps > 0 && !p->a) { *why = "a is NULL"; return PM_EINVAL; }
-    if (p->flags != 0) { *why = "flags must be 0"; return PM_EINVAL; }
+    if (p->flags & ~PM_FLAG_FP64_TRANSFORMS) { *why = "unknown bit in flags"; return PM_EINVAL; }
     if (p->deconvolve != 0 && p->deconvolve != 1) { *why = "deconvolve must be 0 or 1"; return PM_EINVAL; }
     if (p->a) {
         for (int i = 0; i <= p->n_steps; i++) {
@@ -159,7 +159,7 @@ static int scatter_pool_slots(const Geometry &g)
 
 static size_t fft_work_reserve(const Geometry &g) { return 2 * sizeof(float) * (size_t)g.mesh_stride + (32u << 20); }
 
-static size_t carve_workspace(pm_ctx *c, const Geometry &g, void *base)
+static size_t carve_workspace(pm_ctx *c, const Geometry &g, void *base, bool fp64_transforms)
 {
     Carve w(base);
     float *m = w.take<float>((size_t)g.mesh_stride * 7);
@@ -189,7 +189,16 @@ static size_t carve_workspace(pm_ctx *c, const Geometry &g, void *base)
     double *ktab = w.take<double>((size_t)9 * tabn);
     void *ffttab = w.take<char>(fft_own_table_bytes(g));
     void *fftw = w.take<char>(fft_work_reserve(g));
+    double *dm = nullptr;
+    void *fftw64 = nullptr;
+    if (fp64_transforms) {
+        dm = w.take<double>(4 * fft64_mesh_doubles(g));
+        fftw64 = w.take<char>(fft64_work_bytes(g));
+    }
     if (c) {
+        for (int k = 0; k < 4; k++) c->dmesh[k] = dm ? dm + (size_t)k * fft64_mesh_doubles(g) : nullptr;
+        c->fft64_work = fftw64;
+        c->fft64_work_bytes = fp64_transforms ? fft64_work_bytes(g) : 0;
         for (int k = 0; k < 7; k++) c->mesh[k] = m + (size_t)k * g.mesh_stride;
         c->rec = rec; c->offsets = offsets; c->cursor = cursor; c->hist = hist; c->sched = sched; c->wq = wq; c->wq_ints = wq_ints; c->spool_ctl = spool_ctl; c->spool = spool; c->spool_n = spool_n; c->scan_agg = scan_agg;
         c->x = x; c->p = p; c->acc = acc; c->xi = xi; c->pi = pi; c->alpha = alpha;
@@ -318,7 +327,7 @@ int pm_workspace_bytes(const pm_params *params, size_t *bytes)
     if (!bytes) return fail(nullptr, PM_EINVAL, "pm_workspace_bytes", "bytes is NULL");
     int rc = make_geometry(params, &g, &why);
     if (rc != PM_OK) return fail(nullptr, rc, "pm_workspace_bytes", why);
-    *bytes = carve_workspace(nullptr, g, nullptr);
+    *bytes = carve_workspace(nullptr, g, nullptr, (params->flags & PM_FLAG_FP64_TRANSFORMS) != 0);
     return PM_OK;
 }
 
@@ -331,7 +340,8 @@ int pm_init(pm_ctx **out, const pm_params *params, void *dev_workspace, size_t b
     int rc = make_geometry(params, &g, &why);
     if (rc != PM_OK) return fail(nullptr, rc, "pm_init", why);
     if (!dev_workspace || ((uintptr_t)dev_workspace & 255)) return fail(nullptr, PM_EWORKSPACE, "pm_init", "dev_workspace NULL or not 256-byte aligned");
-    size_t need = carve_workspace(nullptr, g, nullptr);
+    const bool f64 = (params->flags & PM_FLAG_FP64_TRANSFORMS) != 0;
+    size_t need = carve_workspace(nullptr, g, nullptr, f64);
     if (bytes < need) return fail(nullptr, PM_EWORKSPACE, "pm_init", "bytes < pm_workspace_bytes");
     pm_ctx *c = new (std::nothrow) pm_ctx();
     if (!c) return fail(nullptr, PM_EINVAL, "pm_init", "out of host memory");
@@ -340,6 +350,8 @@ int pm_init(pm_ctx **out, const pm_params *params, void *dev_workspace, size_t b
     c->prm.a = nullptr;
     c->stream = (cudaStream_t)cuda_stream;
     c->plans_ok = false;
+    c->plans64_ok = false;
+    c->fp64_transforms = f64;
     c->t_index = -1;
     c->have_adjoint = false;
     c->sorted_valid = false;
@@ -358,13 +370,14 @@ int pm_init(pm_ctx **out, const pm_params *params, void *dev_workspace, size_t b
         growth_host(om, c->a[0], gr);
         c->p_over_s0 = gr[2] / gr[0];
     }
-    carve_workspace(c, g, dev_workspace);
+    carve_workspace(c, g, dev_workspace, f64);
     c->tma_ok = false;
-    c->own_fft = fft_own_supported(g);
-    rc = c->own_fft ? PM_OK : make_plans(c);
+    // fp64 transforms go through cuFFT's double-precision plans: the k tables then stay in natural order
+    c->own_fft = !f64 && fft_own_supported(g);
+    rc = f64 ? fft64_init(c) : (c->own_fft ? PM_OK : make_plans(c));
     if (rc == PM_OK) rc = cic_init_tensor_maps(c);
     if (rc == PM_OK) rc = upload_ktab(c);
-    if (rc == PM_OK) rc = fft_own_init(c);
+    if (rc == PM_OK && !f64) rc = fft_own_init(c);
     c->scan_epoch = 0;
     c->wq_epoch = 0;
     if (rc == PM_OK && cudaMemsetAsync(c->wq, 0, sizeof(int) * (size_t)(2 * c->wq_ints), c->stream) != cudaSuccess) rc = fail(c, PM_ECUDA, "pm_init", "clearing the gather work queue");
@@ -414,6 +427,7 @@ int pm_destroy(pm_ctx *c)
 #ifdef PM_DEBUG
     dbg_prec_destroy(c);
 #endif
+    fft64_destroy(c);
     if (c->plans_ok) {
         cufftDestroy(c->plan_r2c1);
         cufftDestroy(c->plan_c2r1);

@@ -84,6 +84,13 @@ struct pm_ctx {
     bool overlap_ok;             // stream2 and the events exist (and PM_OVERLAP != 0)
     cufftHandle plan_r2c1, plan_c2r1;
     bool plans_ok;
+    // PM_FLAG_FP64_TRANSFORMS (pm_fft64.cu): double-precision plans, four fp64 meshes [Nx][Ny][Nz + 2], their work area
+    bool fp64_transforms;
+    cufftHandle plan_d2z, plan_z2d;
+    bool plans64_ok;
+    double *dmesh[4];
+    void *fft64_work;
+    size_t fft64_work_bytes;
     // workspace carve-up (device pointers)
     float *mesh[7];              // padded in-place R2C layout, contiguous
     uint4 *rec;                  // sorted records {X, Y, Z, j}
@@ -232,6 +239,14 @@ int fft_own_init(pm_ctx *c);                                  // needs c->ktab, 
 void fft_own_axis_order(const pm_ctx *c, int axis, std::vector<int> &freq);  // frequency index stored at each memory position
 int fft_own_force(pm_ctx *c, float *rho, float *f3, double nbar, int part = 0);     // part: see pm_fft.cu
 int fft_own_adjoint(pm_ctx *c, float *Pi3, float *psi, double nbar, int part = 0);
+
+// ---- transforms and k-space operators in fp64 (pm_fft64.cu; pm_params.flags bit 0) -----------------------
+size_t fft64_mesh_doubles(const Geometry &g);
+size_t fft64_work_bytes(const Geometry &g);
+int fft64_init(pm_ctx *c);
+void fft64_destroy(pm_ctx *c);
+int fft64_force(pm_ctx *c, const float *rho, float *f3, double nbar);
+int fft64_adjoint(pm_ctx *c, const float *Pi3, float *psi, double nbar);
 
 // ---- integrator elementwise kernels (pm_integrate.cu) -----------------------------------------------
 int state_from_float(pm_ctx *c, const float *s, const float *p);

@@ -32,7 +32,7 @@ def pmlib():
     return binding
 
 
-def test_config1_full_run_against_stored_oracle(pmlib):
+def _config1_run(pmlib, flags):
     gold = np.load(os.path.join(GOLDEN, "run_cfg1.npz"))
     cfg = inputs.config(1)
     s0 = inputs.zeldovich_displacement(cfg["lattice"], cfg["mesh"], seed=1, rms=0.3)
@@ -40,40 +40,66 @@ def test_config1_full_run_against_stored_oracle(pmlib):
     target = inputs.lognormal_target(cfg["mesh"], seed=2, sigma=1.0)
     g = pmlib.host_growth(cfg["omega_m"], cfg["a"][0])
     assert abs(g[2] / g[0] - float(gold["p_over_s"])) <= 1e-8 * float(gold["p_over_s"])
-    pm = pmlib.PM(cfg["mesh"], cfg["lattice"], cfg["omega_m"], cfg["a"])
+    pm = pmlib.PM(cfg["mesh"], cfg["lattice"], cfg["omega_m"], cfg["a"], flags=flags)
     mem0 = torch.cuda.memory_allocated()
     out = pm.run_fwd_adj(*(torch.from_numpy(v).cuda() for v in (s0, p0, target)))
+    # no allocation inside the run: memory independent of the number of steps (PAPER.md L37, L400-402)
+    assert torch.cuda.memory_allocated() - mem0 == sum(v.numel() * 4 for k, v in out.items() if k != "J")
+    pm.close()
+    return gold, s0, out
+
+
+def _gradient_errors(gold, out, k):
+    """rel L2 over the 16384 sampled particles, its value without the worst 1 % of them, median per-particle error"""
+    idx = gold["idx"]
+    a = out[k].cpu().numpy()[idx].astype(np.float64)
+    b = gold[k]
+    e2 = np.sum((a - b) ** 2, axis=1)
+    n2 = np.sum(b ** 2, axis=1)
+    keep = np.argsort(e2)[: int(0.99 * len(e2))]
+    return (float(np.sqrt(e2.sum() / n2.sum())), float(np.sqrt(e2[keep].sum() / n2[keep].sum())),
+            float(np.median(np.sqrt(e2 / n2))))
+
+
+def _check_forward_and_reversal(gold, s0, out):
     idx = gold["idx"]
     s_n = out["s_n"].cpu().numpy()[idx].astype(np.float64)
     rms = float(np.sqrt(np.mean(np.sum((s_n - gold["s_n"]) ** 2, axis=1))))
     assert rms <= 1e-4, f"final positions rms {rms} cell"
     assert rel_l2(out["p_n"].cpu().numpy()[idx], gold["p_n"]) <= 1e-4
     assert abs(out["J"] - float(gold["J"])) <= 1e-4 * abs(float(gold["J"]))
-    # Gradient: the GPU adjoint is the exact discrete adjoint of the GPU's own (bit-reversible) fp32 trajectory; what
-    # separates it from the oracle's is the fp32-vs-fp64 difference of the FORWARD trajectories (1e-5 cell rms here,
-    # the same size as the paper's own fp32 run-to-run deviation, Table 1), amplified by the chaotic motion
-    # inside collapsed regions.  The squared error is carried by a handful of particles (about 20 of the 16384
-    # sampled ones hold 90 % of it), so three numbers are asserted: the plain relative L2 against the paper's own
-    # fp32 adjoint-vs-AD figure (RMSD 4e-5 of sigma 0.015 = 2.7e-3, Fig. 3), and north_star's 1e-3 on the
-    # sample without its worst 1 % of particles and on the median per-particle error.
-    for k in ("xi0", "pi0", "dJ_ds0"):
-        a = out[k].cpu().numpy()[idx].astype(np.float64)
-        b = gold[k]
-        e2 = np.sum((a - b) ** 2, axis=1)
-        n2 = np.sum(b ** 2, axis=1)
-        e = float(np.sqrt(e2.sum() / n2.sum()))
-        keep = np.argsort(e2)[: int(0.99 * len(e2))]
-        e_trim = float(np.sqrt(e2[keep].sum() / n2[keep].sum()))
-        e_med = float(np.median(np.sqrt(e2 / n2)))
-        assert e <= 3e-3, f"{k} rel L2 {e}"
-        assert e_trim <= 1e-3, f"{k} rel L2 without the worst 1% {e_trim}"
-        assert e_med <= 1e-3, f"{k} median per-particle relative error {e_med}"
     # exact reversal of the fixed-point state at full size
     s_q = np.rint(s0.astype(np.float64) * 2.0 ** 32) / 2.0 ** 32
     assert np.array_equal(out["s_rec"].cpu().numpy(), s_q.astype(np.float32))
-    # no allocation inside the run: memory independent of the number of steps (PAPER.md L37, L400-402)
-    assert torch.cuda.memory_allocated() - mem0 == sum(v.numel() * 4 for k, v in out.items() if k != "J")
-    pm.close()
+    return rms
+
+
+def test_config1_full_run_against_stored_oracle(pmlib):
+    """The fp32 path bench.py times.  Positions, momenta, objective and the exact reversal are held to north_star's
+    numbers.  The gradient of THIS path is limited by the fp32 rounding of the 3-D transforms in the forward pass
+    (precision A/B: an fp32 FFT at its theoretical error moves the final positions by 7e-6 cell,
+    and the chaotic motion inside collapsed regions turns that into 1.7e-3 of gradient, carried by a handful of
+    particles); what is asserted here is what the A/B measured with a 1.5x margin, plus the bulk statistics.  The
+    plain 1e-3 bar is asserted on the same run in test_config1_fp32_gradient_at_north_star_bar (last in this file,
+    expected to fail, strict) and met by the fp64-transform mode in the next test."""
+    gold, s0, out = _config1_run(pmlib, 0)
+    _check_forward_and_reversal(gold, s0, out)
+    for k in ("xi0", "pi0", "dJ_ds0"):
+        e, e_trim, e_med = _gradient_errors(gold, out, k)
+        assert e <= 2.6e-3, f"{k} rel L2 {e}"
+        assert e_trim <= 1e-3, f"{k} rel L2 without the worst 1% {e_trim}"
+        assert e_med <= 1e-3, f"{k} median per-particle relative error {e_med}"
+
+
+def test_config1_full_run_fp64_transforms_meets_every_bar(pmlib):
+    """PM_FLAG_FP64_TRANSFORMS (the paper's "more precise floating-point numbers", L371): transforms and k-space
+    operators in fp64, every particle and mesh array still fp32.  North_star's three numbers hold without any trimming."""
+    gold, s0, out = _config1_run(pmlib, pmlib.PM_FLAG_FP64_TRANSFORMS)
+    rms = _check_forward_and_reversal(gold, s0, out)
+    assert rms <= 5e-6
+    for k in ("xi0", "pi0", "dJ_ds0"):
+        e, _, _ = _gradient_errors(gold, out, k)
+        assert e <= 1e-3, f"{k} rel L2 {e}"
 
 
 @pytest.mark.parametrize("order", ["generation", "random"])
@@ -108,3 +134,14 @@ def test_clustered_kernel_inputs_sampled_parity(pmlib, orc, order):
     gs = pm.gather_grad(xd, fd[0].contiguous()).cpu().numpy()
     assert rel_l2(gs[idx], orc.gather_grad(mesh, x[idx], f[0])) <= 1e-5
     pm.close()
+
+
+@pytest.mark.xfail(strict=True, reason="DESIGN.md R27: with fp32 transforms the gradient at configs[1] is 1.7e-3 "
+                   "(precision A/B, section 7); PM_FLAG_FP64_TRANSFORMS meets 1e-3")
+def test_config1_fp32_gradient_at_north_star_bar(pmlib):
+    """north_star's plain 1e-3 on the fp32 path at configs[1], untrimmed.  Kept so that the gap stays visible: it is
+    expected to fail (strict: if the fp32 path ever meets the bar this test turns red and the xfail must go)."""
+    gold, s0, out = _config1_run(pmlib, 0)
+    for k in ("xi0", "pi0", "dJ_ds0"):
+        e, _, _ = _gradient_errors(gold, out, k)
+        assert e <= 1e-3, f"{k} rel L2 {e}"

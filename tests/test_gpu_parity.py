@@ -299,3 +299,35 @@ def test_two_stream_adjoint_step_is_bit_identical(pmlib, orc, monkeypatch):
     assert outs["1"]["J"] == outs["0"]["J"]
     for k in ("s_n", "p_n", "xi0", "pi0", "dJ_ds0", "s_rec", "p_rec"):
         assert torch.equal(outs["1"][k], outs["0"][k]), k
+
+
+@pytest.mark.parametrize("mesh,lattice,deconv", [((24, 20, 36), (12, 10, 18), 1), ((64, 64, 64), (32, 32, 32), 0)])
+def test_fp64_transform_mode_force_and_vjp_parity(pmlib, orc, mesh, lattice, deconv):
+    """PM_FLAG_FP64_TRANSFORMS (include/pm.h): transforms and eq. 11 in fp64, scatter and gathers as in
+    the fp32 mode.  What is left of the difference to the oracle is the gathers' fp32 interpolation: rel L2 <= 2e-6."""
+    rng = np.random.default_rng(23)
+    pm = pmlib.PM(mesh, lattice, 0.3, [0.5, 1.0], deconvolve=deconv, flags=pmlib.PM_FLAG_FP64_TRANSFORMS)
+    s = rng.normal(0, 1.5, (pm.np, 3))
+    x = (orc.positions(mesh, lattice, s)).astype(np.float32)
+    pi = rng.standard_normal((pm.np, 3)).astype(np.float32)
+    acc, alpha = pm.force_vjp(dev(x), dev(pi))
+    assert rel_l2(acc.cpu().numpy(), orc.force(mesh, 0.3, x, deconv=deconv)) <= 2e-6
+    assert rel_l2(alpha.cpu().numpy(), orc.force_vjp(mesh, 0.3, x, pi, deconv=deconv)) <= 2e-6
+    assert pm.workspace_nbytes > pmlib.workspace_bytes(mesh, lattice, 0.3, [0.5, 1.0], deconv)
+    pm.close()
+
+
+def test_fp64_transform_mode_config0_run(pmlib, orc):
+    """the whole forward + adjoint run of configs[0] in the fp64-transform mode: north_star's numbers and exact reversal"""
+    cfg, s0, p0, target = _cfg0_inputs(orc)
+    ref = orc.run_fwd_adj(cfg["mesh"], cfg["lattice"], cfg["omega_m"], cfg["a"], s0, p0, target)
+    pm = pmlib.PM(cfg["mesh"], cfg["lattice"], cfg["omega_m"], cfg["a"], flags=pmlib.PM_FLAG_FP64_TRANSFORMS)
+    out = pm.run_fwd_adj(dev(s0), dev(p0), dev(target))
+    s_n = out["s_n"].cpu().numpy().astype(np.float64)
+    assert np.sqrt(np.mean(np.sum((s_n - ref["s_n"]) ** 2, axis=1))) <= 1e-4
+    assert abs(out["J"] - ref["J"]) <= 1e-4 * abs(ref["J"])
+    for k in ("xi0", "pi0", "dJ_ds0"):
+        assert rel_l2(out[k].cpu().numpy(), ref[k]) <= 1e-3
+    s_q = np.rint(s0.astype(np.float64) * 2.0 ** 32) / 2.0 ** 32
+    assert np.array_equal(out["s_rec"].cpu().numpy(), s_q.astype(np.float32))
+    pm.close()
