@@ -669,3 +669,263 @@ double orc_backprop_storeall(const int N[3], const int L[3], double om, int deco
     free(S); free(p); free(acc); free(x); free(xi); free(pi); free(alpha);
     return J;
 }
+
+/* ------------------------------------------------------------------------------------ */
+/* 7. Initial conditions from white noise by Lagrangian perturbation theory, and the VJP */
+/*    that turns (xi_0, pi_0) into dJ/d(omega)   (eq. 2-6; L406 eq. 51;   */
+/*    growth of second order: L520-555 A1-A8).  SURVEY section 8(f) row 1.                */
+/*                                                                                        */
+/*    omega(q): real white noise on the particle lattice (L89), q_j = j N/L (reading R6). */
+/*    omega(k) = sum_q omega(q) e^{-ik.q}  (L81), k_d = 2 pi m_d / N_d per mesh cell,      */
+/*      m_d in [-L_d/2, L_d/2).                                                           */
+/*    delta1(k) = amp sqrt(P(k)) omega(k), P(k) = k^ns exp(-(rc k)^2), delta1(0) = 0       */
+/*      (eq. 6; the volume factor is part of amp -- DESIGN.md reading R29).               */
+/*    nabla^2 phi1 = delta1  ->  phi1(k) = -delta1(k)/k^2;  s1 = -grad phi1 (eq. 3-4):     */
+/*      s1_d(k) = i kt_d delta1(k)/k^2.                                                   */
+/*    phi1,ab(k) = -k_a k_b phi1(k) = k_a k_b delta1(k)/k^2 ;                              */
+/*    S(q) = sum_{a<b} ( phi1,aa phi1,bb - phi1,ab^2 )  (eq. 4, second line);              */
+/*    nabla^2 phi2 = S -> phi2(k) = -S(k)/k^2 ; s2 = -grad phi2: s2_d(k) = i kt_d S(k)/k^2.*/
+/*    s0 = D1 s1 + D2 s2 ;  p0 = a^2 H (D1' s1 + D2' s2), H = E(a) (H0 = 1)   (eq. 2).     */
+/*    Nyquist planes (reading R10 extended): the odd factors (i kt_d, and k_a k_b with     */
+/*    a != b) are zero where m_d = -L_d/2; the even ones (k^2, k_a^2) are kept.            */
+/* ------------------------------------------------------------------------------------ */
+
+/* right-hand side of eq. A5, both lines (L537), y = (G1, G1', G2, G2'), ' = d/dlna       */
+static void growth2_rhs(double om, double lna, const double y[4], double dy[4])
+{
+    double a = exp(lna);
+    double hh = dlnH_of_a(om, a), oma = Om_of_a(om, a);
+    dy[0] = y[1];
+    dy[1] = -(4.0 + hh) * y[1] - (3.0 + hh - 1.5 * oma) * y[0];
+    dy[2] = y[3];
+    dy[3] = -(6.0 + hh) * y[3] - (8.0 + 2.0 * hh - 1.5 * oma) * y[2] + 1.5 * oma * y[0] * y[0];
+}
+
+/* A5 with the initial conditions A6 (G1 = 1, G1' = 0, G2 = 3/7, G2' = 0 at a = 1e-6),    */
+/* RK4 in ln a as orc_growth.  out = {D2, D2'}: D2 = a^2 G2, D2' = a^2 (2 G2 + G2') (A8,   */
+/* m = 2, garbling corrected as in reading R2).                                           */
+void orc_growth2(double om, double a, double out[2])
+{
+    const double lna0 = log(1e-6), lna1 = log(a);
+    long nstep = (long)ceil((lna1 - lna0) / 1e-3);
+    if (nstep < 1) nstep = 1;
+    double h = (lna1 - lna0) / (double)nstep;
+    double y[4] = {1.0, 0.0, 3.0 / 7.0, 0.0};
+    for (long i = 0; i < nstep; i++) {
+        double t = lna0 + h * (double)i;
+        double k1[4], k2[4], k3[4], k4[4], yt[4];
+        growth2_rhs(om, t, y, k1);
+        for (int c = 0; c < 4; c++) yt[c] = y[c] + 0.5 * h * k1[c];
+        growth2_rhs(om, t + 0.5 * h, yt, k2);
+        for (int c = 0; c < 4; c++) yt[c] = y[c] + 0.5 * h * k2[c];
+        growth2_rhs(om, t + 0.5 * h, yt, k3);
+        for (int c = 0; c < 4; c++) yt[c] = y[c] + h * k3[c];
+        growth2_rhs(om, t + h, yt, k4);
+        for (int c = 0; c < 4; c++) y[c] += h / 6.0 * (k1[c] + 2.0 * k2[c] + 2.0 * k3[c] + k4[c]);
+    }
+    out[0] = a * a * y[2];
+    out[1] = a * a * (2.0 * y[2] + y[3]);
+}
+
+/* lattice mode (ix, iy, iz): k_d (full), kt_d (0 on the lattice Nyquist planes), k^2      */
+static inline void lattice_kvec(const int N[3], const int L[3], int ix, int iy, int iz, double k[3], double kt[3], double *k2)
+{
+    int idx[3] = {ix, iy, iz};
+    double kk = 0.0;
+    for (int d = 0; d < 3; d++) {
+        int m = mode_of(idx[d], L[d]);
+        k[d] = 2.0 * PI_ * (double)m / (double)N[d];
+        kt[d] = (L[d] % 2 == 0 && m == -L[d] / 2) ? 0.0 : k[d];
+        kk += k[d] * k[d];
+    }
+    *k2 = kk;
+}
+
+/* sqrt(P(k)) amp, 0 at k = 0 */
+static inline double ic_transfer(double amp, double ns, double rc, double k2)
+{
+    if (!(k2 > 0.0)) return 0.0;
+    return amp * sqrt(pow(k2, 0.5 * ns) * exp(-rc * rc * k2));
+}
+
+/* multiplier of phi1,ab: k_a k_b / k^2 with the Nyquist rule above; ab = 0..5 for xx yy zz xy xz yz */
+static const int kAB[6][2] = {{0, 0}, {1, 1}, {2, 2}, {0, 1}, {0, 2}, {1, 2}};
+static inline double hess_mult(const double k[3], const double kt[3], double k2, int ab)
+{
+    int a = kAB[ab][0], b = kAB[ab][1];
+    if (!(k2 > 0.0)) return 0.0;
+    return (a == b ? k[a] * k[a] : kt[a] * kt[b]) / k2;
+}
+
+/* real field[np] -> spectrum (new array) ; spectrum -> real part of the inverse transform / np   */
+static cplx *ic_spectrum_of(const int L[3], const double *f)
+{
+    long np = (long)L[0] * L[1] * L[2];
+    cplx *w = (cplx *)malloc(sizeof(cplx) * (size_t)np);
+    for (long i = 0; i < np; i++) w[i] = f[i];
+    orc_fft3d(L[0], L[1], L[2], w, -1);
+    return w;
+}
+static void ic_real_of(const int L[3], cplx *w, double *out, long ostride, double *imag_max)
+{
+    long np = (long)L[0] * L[1] * L[2];
+    orc_fft3d(L[0], L[1], L[2], w, +1);
+    double im = imag_max ? *imag_max : 0.0;
+    for (long i = 0; i < np; i++) {
+        out[i * ostride] = creal(w[i]) / (double)np;
+        double v = fabs(cimag(w[i])) / (double)np;
+        if (v > im) im = v;
+    }
+    if (imag_max) *imag_max = im;
+}
+
+/* s1[3][np], and when order == 2 phi[6][np] (xx yy zz xy xz yz) and s2[3][np], from omega[np] */
+static void ic_fields(const int N[3], const int L[3], double amp, double ns, double rc, int order, const double *omega,
+                      double *s1, double *phi, double *s2, double *imag_max)
+{
+    long np = (long)L[0] * L[1] * L[2];
+    cplx *wk = ic_spectrum_of(L, omega);
+    cplx *t = (cplx *)malloc(sizeof(cplx) * (size_t)np);
+    /* delta1(k) in place */
+    for (int ix = 0; ix < L[0]; ix++) for (int iy = 0; iy < L[1]; iy++) for (int iz = 0; iz < L[2]; iz++) {
+        double k[3], kt[3], k2;
+        lattice_kvec(N, L, ix, iy, iz, k, kt, &k2);
+        wk[((size_t)ix * L[1] + iy) * L[2] + iz] *= ic_transfer(amp, ns, rc, k2);
+    }
+    for (int d = 0; d < 3; d++) {
+        for (int ix = 0; ix < L[0]; ix++) for (int iy = 0; iy < L[1]; iy++) for (int iz = 0; iz < L[2]; iz++) {
+            double k[3], kt[3], k2;
+            size_t o = ((size_t)ix * L[1] + iy) * L[2] + iz;
+            lattice_kvec(N, L, ix, iy, iz, k, kt, &k2);
+            t[o] = k2 > 0.0 ? I * kt[d] / k2 * wk[o] : 0.0;
+        }
+        ic_real_of(L, t, s1 + (size_t)d * np, 1, imag_max);
+    }
+    if (order == 2) {
+        for (int ab = 0; ab < 6; ab++) {
+            for (int ix = 0; ix < L[0]; ix++) for (int iy = 0; iy < L[1]; iy++) for (int iz = 0; iz < L[2]; iz++) {
+                double k[3], kt[3], k2;
+                size_t o = ((size_t)ix * L[1] + iy) * L[2] + iz;
+                lattice_kvec(N, L, ix, iy, iz, k, kt, &k2);
+                t[o] = hess_mult(k, kt, k2, ab) * wk[o];
+            }
+            ic_real_of(L, t, phi + (size_t)ab * np, 1, imag_max);
+        }
+        double *S = (double *)malloc(sizeof(double) * (size_t)np);
+        const double *pxx = phi, *pyy = phi + np, *pzz = phi + 2 * np, *pxy = phi + 3 * np, *pxz = phi + 4 * np, *pyz = phi + 5 * np;
+        for (long i = 0; i < np; i++)
+            S[i] = pxx[i] * pyy[i] + pxx[i] * pzz[i] + pyy[i] * pzz[i] - pxy[i] * pxy[i] - pxz[i] * pxz[i] - pyz[i] * pyz[i];
+        cplx *Sk = ic_spectrum_of(L, S);
+        for (int d = 0; d < 3; d++) {
+            for (int ix = 0; ix < L[0]; ix++) for (int iy = 0; iy < L[1]; iy++) for (int iz = 0; iz < L[2]; iz++) {
+                double k[3], kt[3], k2;
+                size_t o = ((size_t)ix * L[1] + iy) * L[2] + iz;
+                lattice_kvec(N, L, ix, iy, iz, k, kt, &k2);
+                t[o] = k2 > 0.0 ? I * kt[d] / k2 * Sk[o] : 0.0;
+            }
+            ic_real_of(L, t, s2 + (size_t)d * np, 1, imag_max);
+        }
+        free(S); free(Sk);
+    }
+    free(wk); free(t);
+}
+
+/* the four time factors of eq. 2 at a0: {D1, D2, a^2 E D1', a^2 E D2'} */
+void orc_ic_factors(double om, double a0, double out[4])
+{
+    double g1[3], g2[2];
+    orc_growth(om, a0, g1);
+    orc_growth2(om, a0, g2);
+    double a2E = a0 * a0 * sqrt(E2_of_a(om, a0));
+    out[0] = g1[0]; out[1] = g2[0]; out[2] = a2E * g1[1]; out[3] = a2E * g2[1];
+}
+
+/* omega[np] -> s0[np][3], p0[np][3] (eq. 2); order = 1 (Zel'dovich) or 2 (2LPT).          */
+/* Returns the largest |imaginary part| met in any inverse transform (must be rounding).   */
+double orc_ic(const int N[3], const int L[3], double om, double a0, double amp, double ns, double rc, int order,
+              const double *omega, double *s0, double *p0)
+{
+    long np = (long)L[0] * L[1] * L[2];
+    double *s1 = (double *)calloc((size_t)3 * np, sizeof(double)), *s2 = (double *)calloc((size_t)3 * np, sizeof(double));
+    double *phi = (double *)calloc((size_t)6 * np, sizeof(double));
+    double imag_max = 0.0, f[4];
+    ic_fields(N, L, amp, ns, rc, order, omega, s1, phi, s2, &imag_max);
+    orc_ic_factors(om, a0, f);
+    if (order != 2) f[1] = f[3] = 0.0;
+    for (long j = 0; j < np; j++)
+        for (int d = 0; d < 3; d++) {
+            s0[3 * j + d] = f[0] * s1[(size_t)d * np + j] + f[1] * s2[(size_t)d * np + j];
+            p0[3 * j + d] = f[2] * s1[(size_t)d * np + j] + f[3] * s2[(size_t)d * np + j];
+        }
+    free(s1); free(s2); free(phi);
+    return imag_max;
+}
+
+/* transposed multiplier applied to a real field and ACCUMULATED into a spectrum: acc(k) += conj(m(k)) FFT[f](k).   */
+/* kind 0: m = i kt_d / k^2 (component d);  kind 1: m = hess_mult(ab = d)                                          */
+static void ic_accumulate_T(const int N[3], const int L[3], const double *f, int kind, int d, cplx *acc)
+{
+    cplx *w = ic_spectrum_of(L, f);
+    for (int ix = 0; ix < L[0]; ix++) for (int iy = 0; iy < L[1]; iy++) for (int iz = 0; iz < L[2]; iz++) {
+        double k[3], kt[3], k2;
+        size_t o = ((size_t)ix * L[1] + iy) * L[2] + iz;
+        lattice_kvec(N, L, ix, iy, iz, k, kt, &k2);
+        if (!(k2 > 0.0)) continue;
+        if (kind == 0) acc[o] += -I * kt[d] / k2 * w[o];
+        else acc[o] += hess_mult(k, kt, k2, d) * w[o];
+    }
+    free(w);
+}
+
+/* VJP of orc_ic: domega[np] = xi0 . d s0/d omega + pi0 . d p0/d omega  (eq. 51, second line; PAPER.md gives no      */
+/* formula -- "computed by AD", L408 -- so this is the transpose of the steps above, taken one by one, backwards):   */
+/*   c1 = D1 xi0 + (a^2 E D1') pi0, c2 = D2 xi0 + (a^2 E D2') pi0          (cotangents of s1, s2)                    */
+/*   Sbar = sum_d M_d^T c2_d,   M_d = i kt_d / k^2  (real, odd kernel: transpose = conjugate multiplier)             */
+/*   phibar_aa = Sbar (sum_{b != a} phi_bb),  phibar_ab = -2 Sbar phi_ab (a < b)                                     */
+/*   delta1bar = sum_d M_d^T c1_d + sum_ab H_ab^T phibar_ab,   H_ab real and even: its own transpose                 */
+/*   omegabar = T^T delta1bar, T = amp sqrt(P) real and even                                                         */
+void orc_ic_vjp(const int N[3], const int L[3], double om, double a0, double amp, double ns, double rc, int order,
+                const double *omega, const double *xi0, const double *pi0, double *domega)
+{
+    long np = (long)L[0] * L[1] * L[2];
+    double f[4];
+    orc_ic_factors(om, a0, f);
+    cplx *dbar = (cplx *)calloc((size_t)np, sizeof(cplx));      /* delta1bar(k) */
+    double *c = (double *)malloc(sizeof(double) * (size_t)np);
+    for (int d = 0; d < 3; d++) {
+        for (long j = 0; j < np; j++) c[j] = f[0] * xi0[3 * j + d] + f[2] * pi0[3 * j + d];
+        ic_accumulate_T(N, L, c, 0, d, dbar);
+    }
+    if (order == 2) {
+        double *s1 = (double *)calloc((size_t)3 * np, sizeof(double)), *s2 = (double *)calloc((size_t)3 * np, sizeof(double));
+        double *phi = (double *)calloc((size_t)6 * np, sizeof(double));
+        ic_fields(N, L, amp, ns, rc, 2, omega, s1, phi, s2, NULL);      /* phi1,ab of the forward pass */
+        cplx *Sb = (cplx *)calloc((size_t)np, sizeof(cplx));
+        for (int d = 0; d < 3; d++) {
+            for (long j = 0; j < np; j++) c[j] = f[1] * xi0[3 * j + d] + f[3] * pi0[3 * j + d];
+            ic_accumulate_T(N, L, c, 0, d, Sb);
+        }
+        double *Sbar = (double *)malloc(sizeof(double) * (size_t)np);
+        ic_real_of(L, Sb, Sbar, 1, NULL);
+        const double *pxx = phi, *pyy = phi + np, *pzz = phi + 2 * np;
+        for (int ab = 0; ab < 6; ab++) {
+            for (long j = 0; j < np; j++) {
+                double v;
+                if (ab == 0) v = pyy[j] + pzz[j];
+                else if (ab == 1) v = pxx[j] + pzz[j];
+                else if (ab == 2) v = pxx[j] + pyy[j];
+                else v = -2.0 * phi[(size_t)ab * np + j];
+                c[j] = Sbar[j] * v;
+            }
+            ic_accumulate_T(N, L, c, 1, ab, dbar);
+        }
+        free(s1); free(s2); free(phi); free(Sb); free(Sbar);
+    }
+    for (int ix = 0; ix < L[0]; ix++) for (int iy = 0; iy < L[1]; iy++) for (int iz = 0; iz < L[2]; iz++) {
+        double k[3], kt[3], k2;
+        lattice_kvec(N, L, ix, iy, iz, k, kt, &k2);
+        dbar[((size_t)ix * L[1] + iy) * L[2] + iz] *= ic_transfer(amp, ns, rc, k2);
+    }
+    ic_real_of(L, dbar, domega, 1, NULL);
+    free(dbar); free(c);
+}

@@ -79,6 +79,11 @@ def lib():
         L.orc_run_fwd.restype = C.c_double
         L.orc_backprop_storeall.argtypes = [_ip, _ip, C.c_double, C.c_int, C.c_int, _dp] + [_dp] * 5
         L.orc_backprop_storeall.restype = C.c_double
+        L.orc_growth2.argtypes = [C.c_double, C.c_double, _dp]
+        L.orc_ic_factors.argtypes = [C.c_double, C.c_double, _dp]
+        L.orc_ic.argtypes = [_ip, _ip] + [C.c_double] * 5 + [C.c_int, _dp, _dp, _dp]
+        L.orc_ic.restype = C.c_double
+        L.orc_ic_vjp.argtypes = [_ip, _ip] + [C.c_double] * 5 + [C.c_int, _dp, _dp, _dp, _dp]
         _lib = L
     return _lib
 
@@ -274,3 +279,35 @@ def backprop_storeall(N, L, omega_m, a, s0, p0, delta_target, deconv=0):
     J = lib().orc_backprop_storeall(_i3(N), _i3(L), omega_m, deconv, n, _d(a), _d(s0), _d(p0), _d(dt),
                                     _d(xi0), _d(pi0))
     return J, xi0, pi0
+
+
+# ---- initial conditions from white noise (SURVEY 8f row 1; PAPER.md eq. 2-6, eq. 51) ----
+def growth2(omega_m, a):
+    """[D2, dD2/dlna] (eq. A5 second line, A6, A8)."""
+    out = np.zeros(2)
+    lib().orc_growth2(omega_m, a, _d(out))
+    return out
+
+
+def ic_factors(omega_m, a0):
+    """[D1, D2, a^2 E D1', a^2 E D2'] at a0: the four time factors of eq. 2."""
+    out = np.zeros(4)
+    lib().orc_ic_factors(omega_m, a0, _d(out))
+    return out
+
+
+def ic(N, L, omega_m, a0, amp, omega, order=2, ns=-1.5, rc=2.0, return_imag=False):
+    """white noise omega[Lx, Ly, Lz] -> (s0[np, 3], p0[np, 3]) by 1LPT / 2LPT."""
+    om = _f64(omega).reshape(-1)
+    s0 = np.zeros((om.shape[0], 3))
+    p0 = np.zeros_like(s0)
+    im = lib().orc_ic(_i3(N), _i3(L), omega_m, a0, amp, ns, rc, order, _d(om), _d(s0), _d(p0))
+    return (s0, p0, im) if return_imag else (s0, p0)
+
+
+def ic_vjp(N, L, omega_m, a0, amp, omega, xi0, pi0, order=2, ns=-1.5, rc=2.0):
+    """dJ/d omega [np] = xi0 . ds0/domega + pi0 . dp0/domega."""
+    om = _f64(omega).reshape(-1)
+    out = np.zeros_like(om)
+    lib().orc_ic_vjp(_i3(N), _i3(L), omega_m, a0, amp, ns, rc, order, _d(om), _d(_f64(xi0)), _d(_f64(pi0)), _d(out))
+    return out

@@ -255,17 +255,88 @@ __device__ __forceinline__ float mode_green(const GreenCol &c, double k2x, doubl
     return (float)(c.c0 * (decx * c.decyz) * r);
 }
 
-// ---- x pass fused with the force operator: rho(k) -> f_d(k) = i kt_d G rho(k), d = 1..3, back-transformed along x ----
-// grid = (column tiles along z, Ny); shared: spectrum tile + work tile + Nx twiddles + Nx kt_x
-template <int NX, int CS>
-__global__ void __launch_bounds__(FFT_T) fft_x_force_kernel(FftGeom g, const float2 *rho, float2 *f)
+// ---- the fused x kernels: transform along x, k-space operator, back-transform, ONE shared-memory tile ---------------
+// The last forward stage (span RL = its radix, butterflies over RL neighbouring positions) and the first inverse stage
+// work on the same groups of positions, so a thread keeps the outputs of its last-stage butterflies in REGISTERS, applies
+// the operator there and feeds them straight into the first inverse stage(s): the spectrum never goes back to shared
+// memory, and the two back-transforms of the force kernel (f_x, and the common part of f_y, f_z) run one after the other
+// through the same tile.  Half the shared memory of a two-tile design: 8 columns (64-byte pieces) at Nx = 1024 with two
+// CTAs per SM, four CTAs per SM at 512.
+__host__ __device__ constexpr int last_span(int N)
 {
+    int L = N;
+    while (stage_radix(L) != L) L /= stage_radix(L);
+    return L;
+}
+
+// the stages with span > LSTOP only (forward: descending spans, inverse: ascending); every stage is followed by a barrier
+template <int N, int L, bool INV, int PITCH, int CS, int LSTOP>
+struct AxisFFTPartial {
+    static constexpr int R = stage_radix(L);
+    static __device__ __forceinline__ void run(float2 *tile, int ncol, const float2 *tw)
+    {
+        if (!INV) {
+            fft_stage<N, L, false, PITCH, CS>(tile, ncol, tw);
+            __syncthreads();
+            AxisFFTPartial<N, L / R, INV, PITCH, CS, LSTOP>::run(tile, ncol, tw);
+        } else {
+            AxisFFTPartial<N, L / R, INV, PITCH, CS, LSTOP>::run(tile, ncol, tw);
+            fft_stage<N, L, true, PITCH, CS>(tile, ncol, tw);
+            __syncthreads();
+        }
+    }
+};
+template <int N, int LS, bool INV, int PITCH, int CS>
+struct AxisFFTPartial<N, LS, INV, PITCH, CS, LS> {
+    static __device__ __forceinline__ void run(float2 *, int, const float2 *) {}
+};
+
+template <int NX, int CS>
+struct XPlan {
+    static constexpr int B = 1 << CS;
+    static constexpr int RL = last_span(NX);               // span and radix of the last forward / first inverse stage
+    static constexpr int NWORK = (NX / RL) << CS;          // its butterflies per tile
+    static constexpr int IT = (NWORK + FFT_T - 1) / FFT_T; // butterflies per thread: IT * RL spectrum elements in registers
+    // butterfly `it` of this thread: column and first position; false = none (short tile or column beyond ncol)
+    static __device__ __forceinline__ bool item(int it, int ncol, int &col, int &pos0)
+    {
+        const int wk = threadIdx.x + it * FFT_T;
+        col = wk & (B - 1);
+        pos0 = (wk >> CS) * RL;
+        return wk < NWORK && col < ncol;
+    }
+    // last forward stage: X[pos0 + m] of the column, m < RL, in natural order
+    static __device__ __forceinline__ void last_fwd(const float2 *tile, int col, int pos0, float2 (&x)[RL])
+    {
+        float2 v[RL];
+#pragma unroll
+        for (int m = 0; m < RL; m++) v[m] = tile[((pos0 + m) << CS) + col];
+        reg_dft<RL, false>(v);
+#pragma unroll
+        for (int m = 0; m < RL; m++) x[m] = v[bitrev(m, RL)];
+    }
+    // first inverse stage: takes the RL spectrum elements, leaves its outputs in the tile for the remaining stages
+    static __device__ __forceinline__ void first_inv(float2 *tile, int col, int pos0, float2 (&v)[RL])
+    {
+        reg_dft<RL, true>(v);
+#pragma unroll
+        for (int i = 0; i < RL; i++) tile[((pos0 + bitrev(i, RL)) << CS) + col] = v[i];
+    }
+};
+
+#define PM_X_MINBLOCKS(NX) ((NX) >= 1024 ? 2 : ((NX) >= 512 ? 3 : 2))
+
+// ---- x pass fused with the force operator: rho(k) -> f_d(k) = i kt_d G rho(k), d = 1..3, back-transformed along x ----
+// grid = (column tiles along z, Ny); shared: one tile + Nx twiddles + the x-dependent k tables
+template <int NX, int CS>
+__global__ void __launch_bounds__(FFT_T, PM_X_MINBLOCKS(NX)) fft_x_force_kernel(FftGeom g, const float2 *rho, float2 *f)
+{
+    typedef XPlan<NX, CS> P;
+    constexpr int B = P::B, RL = P::RL, IT = P::IT;
     extern __shared__ __align__(16) unsigned char fsm[];
     pdl_trigger();  // the constant tables are loaded before pdl_wait(), the data after it
-    constexpr int B = 1 << CS;
-    float2 *spec = reinterpret_cast<float2 *>(fsm);
-    float2 *work = spec + (NX << CS);
-    float2 *tw = work + (NX << CS);
+    float2 *tile = reinterpret_cast<float2 *>(fsm);
+    float2 *tw = tile + (NX << CS);
     double *k2x = reinterpret_cast<double *>(tw + NX), *decx = k2x + NX;
     float *ktx = reinterpret_cast<float *>(decx + NX);
     const int col0 = blockIdx.x * B, ncol = min(B, g.zsc - col0);
@@ -279,47 +350,63 @@ __global__ void __launch_bounds__(FFT_T) fft_x_force_kernel(FftGeom g, const flo
         decx[i] = g.ktab[2 * g.tabn + i];
     }
     pdl_wait();
-    tile_load<NX, CS>(spec, rho + off, stride, ncol);
+    tile_load<NX, CS>(tile, rho + off, stride, ncol);
     fft_cp_async_wait_all();
     __syncthreads();
-    AxisFFT<NX, NX, false, B, CS>::run(spec, ncol, tw);
-    // Green's function once per mode, in place
-    const int col = threadIdx.x & (B - 1);
-    const int iz = min(col0 + col, g.N[2] / 2);
-    const float kty = (float)g.ktab[3 * g.tabn + iy], ktz = (float)g.ktab[6 * g.tabn + iz];
-    if (col < ncol) {
-        const GreenCol gc = green_col(g, iy, iz);
-#pragma unroll 4
-        for (int pos = threadIdx.x >> CS; pos < NX; pos += FFT_T >> CS) {
-            const float G = mode_green(gc, k2x[pos], decx[pos]);
-            float2 r = spec[(pos << CS) + col];
-            spec[(pos << CS) + col] = make_float2(G * r.x, G * r.y);
+    AxisFFTPartial<NX, NX, false, B, CS, RL>::run(tile, ncol, tw);
+    // last forward stage and Green's function (fp64, rounded once) in registers: h = G rho(k)
+    float2 h[IT][RL];
+    const float kty = (float)g.ktab[3 * g.tabn + iy];
+    {
+        const int colt = threadIdx.x & (B - 1);  // the column of all butterflies of this thread (FFT_T is a multiple of B)
+        const GreenCol gc = green_col(g, iy, min(col0 + colt, g.N[2] / 2));
+#pragma unroll
+        for (int it = 0; it < IT; it++) {
+            int col, pos0;
+            if (!P::item(it, ncol, col, pos0)) continue;
+            P::last_fwd(tile, col, pos0, h[it]);
+#pragma unroll
+            for (int m = 0; m < RL; m++) {
+                const float G = mode_green(gc, k2x[pos0 + m], decx[pos0 + m]);
+                h[it][m] = make_float2(G * h[it][m].x, G * h[it][m].y);
+            }
         }
     }
-    // (no barrier needed: every thread re-reads only the elements it has just written)
-    // kt_y and kt_z do not depend on x, so ONE inverse transform of G rho serves f_y and f_z; f_x needs its own
-    if (col < ncol) {
-#pragma unroll 4
-        for (int pos = threadIdx.x >> CS; pos < NX; pos += FFT_T >> CS) {
-            const float c = ktx[pos];
-            const float2 r = spec[(pos << CS) + col];
-            work[(pos << CS) + col] = make_float2(-c * r.y, c * r.x);  // times +i kt_x
+    // f_x: back-transform of i kt_x h (a thread rewrites only the tile elements it has just read: no barrier before)
+#pragma unroll
+    for (int it = 0; it < IT; it++) {
+        int col, pos0;
+        if (!P::item(it, ncol, col, pos0)) continue;
+        float2 v[RL];
+#pragma unroll
+        for (int m = 0; m < RL; m++) {
+            const float c = ktx[pos0 + m];
+            v[m] = make_float2(-c * h[it][m].y, c * h[it][m].x);
         }
+        P::first_inv(tile, col, pos0, v);
     }
     __syncthreads();
-    AxisFFT<NX, NX, true, B, CS>::run(work, ncol, tw);
-    tile_store<NX, CS>(work, f + off, stride, ncol);
-    AxisFFT<NX, NX, true, B, CS>::run(spec, ncol, tw);
-    // f_y = i kt_y T, f_z = i kt_z T with T = the back-transformed G rho; 16-byte stores of column pairs
+    AxisFFTPartial<NX, NX, true, B, CS, RL>::run(tile, ncol, tw);
+    tile_store<NX, CS>(tile, f + off, stride, ncol);
+    __syncthreads();
+    // kt_y and kt_z do not depend on x, so ONE back-transform T of h serves f_y = i kt_y T and f_z = i kt_z T
+#pragma unroll
+    for (int it = 0; it < IT; it++) {
+        int col, pos0;
+        if (!P::item(it, ncol, col, pos0)) continue;
+        P::first_inv(tile, col, pos0, h[it]);
+    }
+    __syncthreads();
+    AxisFFTPartial<NX, NX, true, B, CS, RL>::run(tile, ncol, tw);
     {
-        constexpr int HB = 1 << (CS - 1);
+        constexpr int HB = 1 << (CS - 1);  // 16-byte stores of column pairs
         const int cp = threadIdx.x & (HB - 1);
         if (2 * cp < ncol) {
             const float kz0 = (float)g.ktab[6 * g.tabn + min(col0 + 2 * cp, g.N[2] / 2)];
             const float kz1 = (float)g.ktab[6 * g.tabn + min(col0 + 2 * cp + 1, g.N[2] / 2)];
 #pragma unroll 4
             for (int pos = threadIdx.x >> (CS - 1); pos < NX; pos += FFT_T >> (CS - 1)) {
-                const float4 t4 = *reinterpret_cast<const float4 *>(spec + (pos << CS) + 2 * cp);
+                const float4 t4 = *reinterpret_cast<const float4 *>(tile + (pos << CS) + 2 * cp);
                 float2 *dst = f + g.cstride + off + (size_t)pos * stride + 2 * cp;
                 *reinterpret_cast<float4 *>(dst) = make_float4(-kty * t4.y, kty * t4.x, -kty * t4.w, kty * t4.z);
                 *reinterpret_cast<float4 *>(dst + g.cstride) = make_float4(-kz0 * t4.y, kz0 * t4.x, -kz1 * t4.w, kz1 * t4.z);
@@ -330,23 +417,21 @@ __global__ void __launch_bounds__(FFT_T) fft_x_force_kernel(FftGeom g, const flo
 
 // ---- x pass fused with the adjoint operator: psi(k) = -i G sum_d kt_d Pi_d(k), back-transformed along x ----------
 template <int NX, int CS>
-__global__ void __launch_bounds__(FFT_T) fft_x_adjoint_kernel(FftGeom g, const float2 *Pi, float2 *psi)
+__global__ void __launch_bounds__(FFT_T, PM_X_MINBLOCKS(NX)) fft_x_adjoint_kernel(FftGeom g, const float2 *Pi, float2 *psi)
 {
+    typedef XPlan<NX, CS> P;
+    constexpr int B = P::B, RL = P::RL, IT = P::IT;
     extern __shared__ __align__(16) unsigned char fsm[];
     pdl_trigger();  // the constant tables are loaded before pdl_wait(), the data after it
-    constexpr int B = 1 << CS;
-    float2 *accum = reinterpret_cast<float2 *>(fsm);
-    float2 *work = accum + (NX << CS);
-    float2 *tw = work + (NX << CS);
+    float2 *tile = reinterpret_cast<float2 *>(fsm);
+    float2 *tw = tile + (NX << CS);
     double *k2x = reinterpret_cast<double *>(tw + NX), *decx = k2x + NX;
     float *ktx = reinterpret_cast<float *>(decx + NX);
     const int col0 = blockIdx.x * B, ncol = min(B, g.zsc - col0);
     const int iy = blockIdx.y;
     const long long stride = (long long)g.N[1] * g.zsc;
     const size_t off = (size_t)iy * g.zsc + col0;
-    const int col = threadIdx.x & (B - 1);
-    const int iz = min(col0 + col, g.N[2] / 2);
-    const float kty = (float)g.ktab[3 * g.tabn + iy], ktz = (float)g.ktab[6 * g.tabn + iz];
+    const float kty = (float)g.ktab[3 * g.tabn + iy];
     load_tw(tw, g.twx, NX);
     for (int i = threadIdx.x; i < NX; i += FFT_T) {
         ktx[i] = (float)g.ktab[i];
@@ -354,39 +439,62 @@ __global__ void __launch_bounds__(FFT_T) fft_x_adjoint_kernel(FftGeom g, const f
         decx[i] = g.ktab[2 * g.tabn + i];
     }
     pdl_wait();
+    // Pi_x: transform along x, spectrum kept in registers
+    tile_load<NX, CS>(tile, Pi + off, stride, ncol);
+    fft_cp_async_wait_all();
+    __syncthreads();
+    AxisFFTPartial<NX, NX, false, B, CS, RL>::run(tile, ncol, tw);
+    float2 hx[IT][RL];
+#pragma unroll
+    for (int it = 0; it < IT; it++) {
+        int col, pos0;
+        if (!P::item(it, ncol, col, pos0)) continue;
+        P::last_fwd(tile, col, pos0, hx[it]);
+    }
+    __syncthreads();  // the tile is refilled by other threads
     // kt_y and kt_z do not depend on x: kt_y Pi_y + kt_z Pi_z is formed BEFORE the transform along x, so two forward
     // transforms (Pi_x and that sum) instead of three
-    tile_load<NX, CS>(accum, Pi + g.cstride + off, stride, ncol);
-    tile_load<NX, CS>(work, Pi + 2 * g.cstride + off, stride, ncol);
-    fft_cp_async_wait_all();
-    __syncthreads();
-    if (col < ncol) {
+    {
+        constexpr int HB = 1 << (CS - 1);
+        const int cp = threadIdx.x & (HB - 1);
+        if (2 * cp < ncol) {
+            const float kz0 = (float)g.ktab[6 * g.tabn + min(col0 + 2 * cp, g.N[2] / 2)];
+            const float kz1 = (float)g.ktab[6 * g.tabn + min(col0 + 2 * cp + 1, g.N[2] / 2)];
+            const float2 *py = Pi + g.cstride + off + 2 * cp, *pz = py + g.cstride;
 #pragma unroll 4
-        for (int pos = threadIdx.x >> CS; pos < NX; pos += FFT_T >> CS) {
-            const float2 vy = accum[(pos << CS) + col], vz = work[(pos << CS) + col];
-            accum[(pos << CS) + col] = make_float2(kty * vy.x + ktz * vz.x, kty * vy.y + ktz * vz.y);
+            for (int pos = threadIdx.x >> (CS - 1); pos < NX; pos += FFT_T >> (CS - 1)) {
+                const float4 a = __ldg(reinterpret_cast<const float4 *>(py + (size_t)pos * stride));
+                const float4 b = __ldg(reinterpret_cast<const float4 *>(pz + (size_t)pos * stride));
+                *reinterpret_cast<float4 *>(tile + (pos << CS) + 2 * cp) =
+                    make_float4(kty * a.x + kz0 * b.x, kty * a.y + kz0 * b.y, kty * a.z + kz1 * b.z, kty * a.w + kz1 * b.w);
+            }
         }
     }
     __syncthreads();
-    tile_load<NX, CS>(work, Pi + off, stride, ncol);
-    AxisFFT<NX, NX, false, B, CS>::run(accum, ncol, tw);
-    fft_cp_async_wait_all();
-    __syncthreads();
-    AxisFFT<NX, NX, false, B, CS>::run(work, ncol, tw);
-    if (col < ncol) {
-        const GreenCol gc = green_col(g, iy, iz);
-#pragma unroll 4
-        for (int pos = threadIdx.x >> CS; pos < NX; pos += FFT_T >> CS) {
-            const float c = ktx[pos];
-            const float2 v = work[(pos << CS) + col], a = accum[(pos << CS) + col];
-            const float G = mode_green(gc, k2x[pos], decx[pos]);
-            // times -i G: (re, im) -> (G im, -G re)
-            accum[(pos << CS) + col] = make_float2(G * (c * v.y + a.y), -G * (c * v.x + a.x));
+    AxisFFTPartial<NX, NX, false, B, CS, RL>::run(tile, ncol, tw);
+    {
+        const int colt = threadIdx.x & (B - 1);
+        const GreenCol gc = green_col(g, iy, min(col0 + colt, g.N[2] / 2));
+#pragma unroll
+        for (int it = 0; it < IT; it++) {
+            int col, pos0;
+            if (!P::item(it, ncol, col, pos0)) continue;
+            float2 a[RL];
+            P::last_fwd(tile, col, pos0, a);
+#pragma unroll
+            for (int m = 0; m < RL; m++) {
+                const float c = ktx[pos0 + m];
+                const float G = mode_green(gc, k2x[pos0 + m], decx[pos0 + m]);
+                const float2 v = hx[it][m];
+                // times -i G: (re, im) -> (G im, -G re)
+                a[m] = make_float2(G * (c * v.y + a[m].y), -G * (c * v.x + a[m].x));
+            }
+            P::first_inv(tile, col, pos0, a);
         }
     }
     __syncthreads();
-    AxisFFT<NX, NX, true, B, CS>::run(accum, ncol, tw);
-    tile_store<NX, CS>(accum, psi + off, stride, ncol);
+    AxisFFTPartial<NX, NX, true, B, CS, RL>::run(tile, ncol, tw);
+    tile_store<NX, CS>(tile, psi + off, stride, ncol);
 }
 
 // ---- z pass, real -> half-complex, in place on ZROWS consecutive z-rows per CTA ---------------------------------
@@ -639,7 +747,7 @@ int fft_own_init(pm_ctx *c)
         case 128: CASE(128, 4); break;  \
         case 256: CASE(256, 4); break;  \
         case 512: CASE(512, 3); break;  \
-        case 1024: CASE(1024, 2); break; \
+        case 1024: CASE(1024, 3); break; \
         default: return fail(c, PM_EINVAL, "own FFT", "unsupported axis length"); \
     }
 #define PM_FFT_SWITCH(n, CASE)          \
@@ -707,9 +815,9 @@ static int fft_x_fused(pm_ctx *c, const float *in, float *out, double nbar, bool
     const Geometry &g = c->g;
     FftGeom fg = *geom_of(c);
     fg.c0 = 1.5 * c->prm.omega_m / (nbar * (double)g.ng);
-    const int cs = g.N[0] <= 256 ? 4 : (g.N[0] <= 512 ? 3 : 2), B = 1 << cs;  // two tiles of Nx x B: keep 3 CTAs per SM
+    const int cs = g.N[0] <= 256 ? 4 : 3, B = 1 << cs;  // one tile of Nx x B: 64-byte pieces at 512 and 1024
     dim3 grid((unsigned)((fg.zsc + B - 1) / B), (unsigned)g.N[1]);
-    size_t smem = sizeof(float2) * ((size_t)g.N[0] + 2 * (size_t)g.N[0] * B) + (2 * sizeof(double) + sizeof(float)) * (size_t)g.N[0];
+    size_t smem = sizeof(float2) * ((size_t)g.N[0] + (size_t)g.N[0] * B) + (2 * sizeof(double) + sizeof(float)) * (size_t)g.N[0];
     Timer t(c, adjoint ? TC_KSPACE_ADJ : TC_KSPACE_FORCE, 32.0 * (double)g.nk);
 #define X_CASE(NN, CS_)                                                                                                                   \
     if (adjoint) PM_FFT_LAUNCH(c, "fft_x_adjoint_kernel", (fft_x_adjoint_kernel<NN, CS_>), grid, smem, fg, (const float2 *)in, (float2 *)out); \
