@@ -155,6 +155,21 @@ int pm_run_fwd_adj_host(pm_ctx *ctx, const float *host_s0, const float *host_p0,
                         const float *host_delta_target, float *host_s_n, float *host_p_n, double *host_J,
                         float *host_xi0, float *host_pi0, float *host_dJ_ds0, float *host_s_rec, float *host_p_rec);
 
+/* ---- initial conditions from white noise, and dJ/d(omega) (eq. 2-6; eq. 51 second line L406) ----------------
+ * dev_omega[Lx][Ly][Lz]: real white noise on the particle lattice (L89).  delta_1(k) = amp sqrt(P(k)) omega(k) with
+ * P(k) = k^ns exp(-(rc k)^2), k in radians per mesh cell (eq. 6; the volume factor is part of amp; the configs' recipe is
+ * ns = -1.5, rc = 2).  order 1: s0 = D1 s1, p0 = a^2 H D1' s1 (Zel'dovich); order 2 adds D2 s2, a^2 H D2' s2 (2LPT, eq. 2-4)
+ * at a_0 = the ctx's first scale factor.  Transforms run on the lattice (cuFFT), the multipliers in fp64 per mode.
+ * Both calls use the ctx's mesh buffers as scratch: call them outside a run (the integrator state is invalidated;
+ * pm_set_state / pm_run_fwd_adj start a new one).  Outputs dev_s0, dev_p0 [N_p][3]; dev_domega [Lx][Ly][Lz]. */
+int pm_ic_fwd(pm_ctx *ctx, const float *dev_omega, double amp, double ns, double rc, int order, float *dev_s0,
+              float *dev_p0);
+/* dev_domega = xi0 . d s0 / d omega + pi0 . d p0 / d omega: with (xi0, pi0) of pm_run_fwd_adj this is dJ/d omega. */
+int pm_ic_vjp(pm_ctx *ctx, const float *dev_omega, double amp, double ns, double rc, int order, const float *dev_xi0,
+              const float *dev_pi0, float *dev_domega);
+/* Host: out = {D1, D2, a^2 E D1', a^2 E D2'} at a0, the four time factors of eq. 2 (D2 by RK4 on eq. A1). */
+int pm_host_ic_factors(double omega_m, double a0, double out[4]);
+
 /* ---- instrumentation ---------------------------------------------------------------------------------
  * When enabled, every kernel launch / cuFFT call of the library is bracketed by CUDA events on the
  * ctx's stream.  pm_timing_read SYNCHRONISES, sums the elapsed time per kernel class since the last

@@ -52,6 +52,9 @@ _SIGS = {
     "pm_host_step_factors": (_int, [_dbl, _dbl, _dbl, C.POINTER(_dbl)]),
     "pm_step_factors": (_int, [_vp, _int, C.POINTER(_dbl)]),
     "pm_host_fft_order": (_int, [C.c_int32, C.POINTER(C.c_int32)]),
+    "pm_host_ic_factors": (_int, [_dbl, _dbl, C.POINTER(_dbl)]),
+    "pm_ic_fwd": (_int, [_vp, _vp, _dbl, _dbl, _dbl, _int, _vp, _vp]),
+    "pm_ic_vjp": (_int, [_vp, _vp, _dbl, _dbl, _dbl, _int, _vp, _vp, _vp]),
     "pm_scatter": (_int, [_vp, _i64, _vp, _vp, _int, _vp]),
     "pm_gather": (_int, [_vp, _i64, _vp, _vp, _int, _vp]),
     "pm_gather_grad": (_int, [_vp, _i64, _vp, _vp, _int, _vp, _vp]),
@@ -115,6 +118,15 @@ def host_step_factors(omega_m, a_prev, a_next):
     rc = _lib.pm_host_step_factors(float(omega_m), float(a_prev), float(a_next), out)
     if rc != PM_OK:
         raise PMError(rc, "pm_host_step_factors")
+    return list(out)
+
+
+def host_ic_factors(omega_m, a0):
+    """[D1, D2, a^2 E D1', a^2 E D2'] at a0: the time factors of eq. 2 (pure host)."""
+    out = (_dbl * 4)()
+    rc = _lib.pm_host_ic_factors(float(omega_m), float(a0), out)
+    if rc != PM_OK:
+        raise PMError(rc, "pm_host_ic_factors")
     return list(out)
 
 
@@ -237,6 +249,21 @@ class PM:
         alpha = self._new(x.shape[0], 3)
         self._call(_lib.pm_force_vjp, x.shape[0], _ptr(x, "x"), _ptr(pi, "pi"), acc.data_ptr(), alpha.data_ptr())
         return acc, alpha
+
+    # ---- initial conditions (eq. 2-6) and dJ/d(omega) (eq. 51) ----
+    def ic_fwd(self, omega, amp, order=2, ns=-1.5, rc=2.0):
+        """white noise omega[Lx, Ly, Lz] -> (s0, p0) [N_p, 3] at the ctx's first scale factor"""
+        s0, p0 = self._new(self.np, 3), self._new(self.np, 3)
+        self._check(_lib.pm_ic_fwd(self._h, _ptr(omega, "omega"), float(amp), float(ns), float(rc), int(order),
+                                   s0.data_ptr(), p0.data_ptr()), "pm_ic_fwd")
+        return s0, p0
+
+    def ic_vjp(self, omega, amp, xi0, pi0, order=2, ns=-1.5, rc=2.0):
+        """dJ/d omega [Lx, Ly, Lz] from the adjoint run's (xi0, pi0)"""
+        out = torch.empty(self.lattice, dtype=torch.float32, device=self.device)
+        self._check(_lib.pm_ic_vjp(self._h, _ptr(omega, "omega"), float(amp), float(ns), float(rc), int(order),
+                                   _ptr(xi0, "xi0"), _ptr(pi0, "pi0"), out.data_ptr()), "pm_ic_vjp")
+        return out
 
     # ---- integrator ----
     def set_state(self, s, p):

@@ -351,6 +351,7 @@ int pm_init(pm_ctx **out, const pm_params *params, void *dev_workspace, size_t b
     c->stream = (cudaStream_t)cuda_stream;
     c->plans_ok = false;
     c->plans64_ok = false;
+    c->plans_ic_ok = false;
     c->fp64_transforms = f64;
     c->t_index = -1;
     c->have_adjoint = false;
@@ -428,6 +429,7 @@ int pm_destroy(pm_ctx *c)
     dbg_prec_destroy(c);
 #endif
     fft64_destroy(c);
+    ic_destroy(c);
     if (c->plans_ok) {
         cufftDestroy(c->plan_r2c1);
         cufftDestroy(c->plan_c2r1);

@@ -85,6 +85,8 @@ struct pm_ctx {
     cufftHandle plan_r2c1, plan_c2r1;
     bool plans_ok;
     // PM_FLAG_FP64_TRANSFORMS (pm_fft64.cu): double-precision plans, four fp64 meshes [Nx][Ny][Nz + 2], their work area
+    cufftHandle plan_ic_r2c, plan_ic_c2r;   // transforms on the particle lattice (pm_ic.cu), created at the first pm_ic_* call
+    bool plans_ic_ok;
     bool fp64_transforms;
     cufftHandle plan_d2z, plan_z2d;
     bool plans64_ok;
@@ -247,6 +249,9 @@ int fft64_init(pm_ctx *c);
 void fft64_destroy(pm_ctx *c);
 int fft64_force(pm_ctx *c, const float *rho, float *f3, double nbar);
 int fft64_adjoint(pm_ctx *c, const float *Pi3, float *psi, double nbar);
+
+// ---- initial conditions (pm_ic.cu) ---------------------------------------------------------------------
+void ic_destroy(pm_ctx *c);
 
 // ---- integrator elementwise kernels (pm_integrate.cu) -----------------------------------------------
 int state_from_float(pm_ctx *c, const float *s, const float *p);

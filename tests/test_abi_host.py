@@ -116,3 +116,13 @@ def test_own_fft_memory_order_is_the_dif_digit_reversal(binding):
         assert np.allclose(y, ref[order], rtol=1e-10, atol=1e-10), n
     with pytest.raises(binding.PMError):
         binding.host_fft_order(48)
+
+
+def test_host_ic_factors_match_the_oracle_by_another_route():
+    """pm_host_ic_factors integrates eq. A1 in D (RK4), the oracle eq. A5 in G: D2, D2' agree; EdS closed form (A3)."""
+    from oracle import pm_oracle as orc
+    from paper_2211_09815_b200 import binding
+    for om, a0 in ((1.0, 0.25), (0.3, 1.0 / 64), (0.3, 0.5)):
+        np.testing.assert_allclose(binding.host_ic_factors(om, a0), orc.ic_factors(om, a0), rtol=3e-8)
+    f = binding.host_ic_factors(1.0, 0.25)
+    np.testing.assert_allclose(f, [0.25, 3 / 7 * 0.0625, 0.25 ** 1.5, 6 / 7 * 0.25 ** 2.5], rtol=1e-9)
