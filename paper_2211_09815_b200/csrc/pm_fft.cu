@@ -98,6 +98,15 @@ __host__ __device__ constexpr int stage_radix(int L)
     return L >= 16 ? (lg % 4 == 1 ? 8 : 16) : L;
 }
 
+// ---- bank-conflict-free rows of 8 columns ------------------------------------------------------------------
+// A tile row of 8 float2 columns (64 bytes) covers half of the 32 banks: even rows one half, odd rows the other.  The
+// stages whose butterflies sit 4 rows apart (the last radix-4 stage; the stage of span 64 of the 512 / 1024 plans) then
+// find all rows of a warp request in the same half (ncu: 25-32 % of the shared-memory wavefronts of the y and x passes
+// at 512 were bank conflicts).  Rows are therefore stored at row ^ bit 2 of the row: consecutive rows still alternate
+// halves, and so do rows 4 apart.  Tiles of 16 columns (128-byte rows) and the padded z tiles need none of this.
+template <bool SWZ>
+__device__ __forceinline__ int trow(int pos) { return SWZ ? pos ^ ((pos >> 2) & 1) : pos; }
+
 // ---- one transform along the tile's position axis, everything but the data known at compile time -----------
 // tile [N][PITCH] (float2), columns [0, ncol) of 1 << CS; tw = exp(-2 pi i k / N), k < N (shared memory).
 // Stage of span L, radix R = stage_radix(L): butterfly (blk, j) takes positions blk L + j + m L/R, m < R.
@@ -107,16 +116,19 @@ __device__ __forceinline__ void fft_stage(float2 *tile, int ncol, const float2 *
     constexpr int R = stage_radix(L);
     constexpr int Lr = L / R, twstep = N / L;
     constexpr int nwork = (N / R) << CS;
+    constexpr bool SWZ = CS == 3 && PITCH == 8;      // rows of 8 unpadded columns: see trow()
+    constexpr bool SAME = !SWZ || Lr % 8 == 0;        // every element of a butterfly gets the same row swizzle
 #pragma unroll 1
     for (int wk = threadIdx.x; wk < nwork; wk += FFT_T) {
         const int col = wk & ((1 << CS) - 1);
         if (col >= ncol) continue;
         const int bf = wk >> CS;
         const int blk = bf / Lr, j = bf - blk * Lr;
-        float2 *p = tile + (blk * L + j) * PITCH + col;
+        const int base = blk * L + j;
+        float2 *p = tile + (SAME ? trow<SWZ>(base) : base) * PITCH + col;
         float2 v[R];
 #pragma unroll
-        for (int m = 0; m < R; m++) v[m] = p[m * Lr * PITCH];
+        for (int m = 0; m < R; m++) v[m] = SAME ? p[m * Lr * PITCH] : tile[trow<SWZ>(base + m * Lr) * PITCH + col];
         if (INV && Lr > 1) {
 #pragma unroll
             for (int q = 1; q < R; q++) v[q] = cmulc(v[q], tw[j * q * twstep]);
@@ -127,7 +139,8 @@ __device__ __forceinline__ void fft_stage(float2 *tile, int ncol, const float2 *
             const int q = bitrev(i, R);
             float2 o = v[i];
             if (!INV && Lr > 1 && q != 0) o = cmul(o, tw[j * q * twstep]);
-            p[q * Lr * PITCH] = o;
+            if (SAME) p[q * Lr * PITCH] = o;
+            else tile[trow<SWZ>(base + q * Lr) * PITCH + col] = o;
         }
     }
 }
@@ -191,7 +204,7 @@ __device__ __forceinline__ void tile_load(float2 *tile, const float2 *base, long
     if (2 * cp < ncol) {
 #pragma unroll 4
         for (int pos = threadIdx.x >> (CS - 1); pos < N; pos += FFT_T >> (CS - 1))
-            fft_cp_async16(tile + (pos << CS) + 2 * cp, base + (size_t)pos * stride + 2 * cp);
+            fft_cp_async16(tile + (trow<CS == 3>(pos) << CS) + 2 * cp, base + (size_t)pos * stride + 2 * cp);
     }
 }
 template <int N, int CS>
@@ -202,7 +215,7 @@ __device__ __forceinline__ void tile_store(const float2 *tile, float2 *base, lon
     if (2 * cp < ncol) {
 #pragma unroll 4
         for (int pos = threadIdx.x >> (CS - 1); pos < N; pos += FFT_T >> (CS - 1))
-            *reinterpret_cast<float4 *>(base + (size_t)pos * stride + 2 * cp) = *reinterpret_cast<const float4 *>(tile + (pos << CS) + 2 * cp);
+            *reinterpret_cast<float4 *>(base + (size_t)pos * stride + 2 * cp) = *reinterpret_cast<const float4 *>(tile + (trow<CS == 3>(pos) << CS) + 2 * cp);
     }
 }
 __device__ __forceinline__ void load_tw(float2 *dst, const float2 *src, int n)
@@ -310,7 +323,7 @@ struct XPlan {
     {
         float2 v[RL];
 #pragma unroll
-        for (int m = 0; m < RL; m++) v[m] = tile[((pos0 + m) << CS) + col];
+        for (int m = 0; m < RL; m++) v[m] = tile[(trow<CS == 3>(pos0 + m) << CS) + col];
         reg_dft<RL, false>(v);
 #pragma unroll
         for (int m = 0; m < RL; m++) x[m] = v[bitrev(m, RL)];
@@ -320,7 +333,7 @@ struct XPlan {
     {
         reg_dft<RL, true>(v);
 #pragma unroll
-        for (int i = 0; i < RL; i++) tile[((pos0 + bitrev(i, RL)) << CS) + col] = v[i];
+        for (int i = 0; i < RL; i++) tile[(trow<CS == 3>(pos0 + bitrev(i, RL)) << CS) + col] = v[i];
     }
 };
 
@@ -406,7 +419,7 @@ __global__ void __launch_bounds__(FFT_T, PM_X_MINBLOCKS(NX)) fft_x_force_kernel(
             const float kz1 = (float)g.ktab[6 * g.tabn + min(col0 + 2 * cp + 1, g.N[2] / 2)];
 #pragma unroll 4
             for (int pos = threadIdx.x >> (CS - 1); pos < NX; pos += FFT_T >> (CS - 1)) {
-                const float4 t4 = *reinterpret_cast<const float4 *>(tile + (pos << CS) + 2 * cp);
+                const float4 t4 = *reinterpret_cast<const float4 *>(tile + (trow<CS == 3>(pos) << CS) + 2 * cp);
                 float2 *dst = f + g.cstride + off + (size_t)pos * stride + 2 * cp;
                 *reinterpret_cast<float4 *>(dst) = make_float4(-kty * t4.y, kty * t4.x, -kty * t4.w, kty * t4.z);
                 *reinterpret_cast<float4 *>(dst + g.cstride) = make_float4(-kz0 * t4.y, kz0 * t4.x, -kz1 * t4.w, kz1 * t4.z);
@@ -465,7 +478,7 @@ __global__ void __launch_bounds__(FFT_T, PM_X_MINBLOCKS(NX)) fft_x_adjoint_kerne
             for (int pos = threadIdx.x >> (CS - 1); pos < NX; pos += FFT_T >> (CS - 1)) {
                 const float4 a = __ldg(reinterpret_cast<const float4 *>(py + (size_t)pos * stride));
                 const float4 b = __ldg(reinterpret_cast<const float4 *>(pz + (size_t)pos * stride));
-                *reinterpret_cast<float4 *>(tile + (pos << CS) + 2 * cp) =
+                *reinterpret_cast<float4 *>(tile + (trow<CS == 3>(pos) << CS) + 2 * cp) =
                     make_float4(kty * a.x + kz0 * b.x, kty * a.y + kz0 * b.y, kty * a.z + kz1 * b.z, kty * a.w + kz1 * b.w);
             }
         }
@@ -497,10 +510,16 @@ __global__ void __launch_bounds__(FFT_T, PM_X_MINBLOCKS(NX)) fft_x_adjoint_kerne
     tile_store<NX, CS>(tile, psi + off, stride, ncol);
 }
 
-// ---- z pass, real -> half-complex, in place on ZROWS consecutive z-rows per CTA ---------------------------------
+// ---- z pass, real -> half-complex, in place on ZROWS consecutive z-rows per CTA, ONE tile ---------------------------
 // row = [zs floats] -> [zsc complex]; x_n real, n < Nz = 2M: z_n = x_2n + i x_2n+1, Z = FFT_M(z),
-// E_k = (Z_k + conj Z_{M-k}) / 2, O_k = (Z_k - conj Z_{M-k}) / (2i), X_k = E_k + w^k O_k, w = e^{-2 pi i / Nz}, k = 0..M
-// shared: tile [M][ZP] + out [M + 1][ZP] + M twiddles + (M + 1) post twiddles + M positions
+// E_k = (Z_k + conj Z_{M-k}) / 2, O_k = (Z_k - conj Z_{M-k}) / (2i), X_k = E_k + w^k O_k, w = e^{-2 pi i / Nz}, k = 0..M,
+// and X_{M-k} = conj(E_k - w^k O_k): one thread turns the pair (Z_k, Z_{M-k}) into (X_k, X_{M-k}) IN PLACE.
+// The rows go straight from global memory into the transposed tile [position][row] and back (a warp moves 32 consecutive
+// elements of one row: coalesced; the odd tile pitch keeps the strided shared-memory side free of bank conflicts), so
+// there is neither a staging buffer nor a second tile.  The spectrum is left in the tile's own order: column p < M of a
+// row holds the frequency the forward stages leave at position p (digit-reversed, as along x and y), column M the Nyquist
+// frequency; only the k tables know (R26).
+// shared: tile [M + 1][ZP] + M twiddles + (M/2 + 1) post twiddles + M positions
 template <int M, int ZRS>
 __global__ void __launch_bounds__(FFT_T) fft_z_r2c_kernel(FftGeom g, float *data, long long nrows)
 {
@@ -508,59 +527,53 @@ __global__ void __launch_bounds__(FFT_T) fft_z_r2c_kernel(FftGeom g, float *data
     extern __shared__ __align__(16) unsigned char fsm[];
     pdl_trigger();  // the constant tables are loaded before pdl_wait(), the data after it
     float2 *tile = reinterpret_cast<float2 *>(fsm);
-    float2 *outb = tile + M * ZP;
-    float2 *tw = outb + max((M + 1) * ZP, ZROWS * g.zsc);
+    float2 *tw = tile + (M + 1) * ZP;
     float2 *twr = tw + M;
-    int *posz = reinterpret_cast<int *>(twr + (M + 1));
-    const int zs = 2 * g.zsc;
+    int *posz = reinterpret_cast<int *>(twr + (M / 2 + 1));
+    const int zsc = g.zsc;
     const long long row0 = (long long)blockIdx.x * ZROWS;
     const int nr = (int)min((long long)ZROWS, nrows - row0);
-    float *rows = data + (size_t)row0 * zs;
-    // the nr rows are contiguous in memory: 16-byte async copies into a row-major staging area (which shares its
-    // shared memory with outb), then the transposing fill of the tile
-    float *stage = reinterpret_cast<float *>(outb);
+    float2 *rows = reinterpret_cast<float2 *>(data) + (size_t)row0 * zsc;
     load_tw(tw, g.twz, M);
-    load_tw(twr, g.twzr, M + 1);
+    load_tw(twr, g.twzr, M / 2 + 1);
     for (int i = threadIdx.x; i < M; i += FFT_T) posz[i] = g.posz[i];
     pdl_wait();
-    {
-        const int nchunk = nr * (zs / 4);
-        for (int i = threadIdx.x; i < nchunk; i += FFT_T) fft_cp_async16(stage + 4 * i, rows + 4 * (size_t)i);
-    }
-    fft_cp_async_wait_all();
-    __syncthreads();
-    {
-        const int r = threadIdx.x & (ZROWS - 1);
-        if (r < nr) {
-#pragma unroll 4
-            for (int n = threadIdx.x >> ZRS; n < M; n += FFT_T >> ZRS) tile[n * ZP + r] = *reinterpret_cast<const float2 *>(stage + r * (2 * M + 4) + 2 * n);
-        }
+#pragma unroll 8
+    for (int idx = threadIdx.x; idx < M * ZROWS; idx += FFT_T) {
+        const int n = idx & (M - 1), r = idx / M;
+        if (r < nr) tile[n * ZP + r] = __ldg(rows + (size_t)r * zsc + n);
     }
     __syncthreads();
     AxisFFT<M, M, false, ZP, ZRS>::run(tile, nr, tw);
-
-    {
-        const int r = threadIdx.x & (ZROWS - 1);
-        if (r < nr) {
-#pragma unroll 4
-            for (int k = threadIdx.x >> ZRS; k <= M; k += FFT_T >> ZRS) {
-                const int km = k == M ? 0 : k, kc = (k == 0 || k == M) ? 0 : M - k;
-                const float2 a = tile[posz[km] * ZP + r], b = tile[posz[kc] * ZP + r];
-                const float2 E = make_float2(0.5f * (a.x + b.x), 0.5f * (a.y - b.y));
-                const float2 O = make_float2(0.5f * (a.y + b.y), -0.5f * (a.x - b.x));  // (a - conj b) / (2i)
-                outb[k * ZP + r] = cadd(E, cmul(twr[k], O));
-            }
+    for (int w = threadIdx.x; w < (M / 2 + 1) * ZROWS; w += FFT_T) {
+        const int r = w & (ZROWS - 1), k = w >> ZRS;
+        if (r >= nr) continue;
+        float2 *pa = tile + posz[k] * ZP + r;
+        const float2 a = *pa;
+        if (k == 0) {
+            *pa = make_float2(a.x + a.y, 0.f);
+            tile[M * ZP + r] = make_float2(a.x - a.y, 0.f);
+        } else if (2 * k == M) {
+            *pa = make_float2(a.x, -a.y);
+        } else {
+            float2 *pb = tile + posz[M - k] * ZP + r;
+            const float2 b = *pb;
+            const float2 E = make_float2(0.5f * (a.x + b.x), 0.5f * (a.y - b.y));
+            const float2 O = make_float2(0.5f * (a.y + b.y), -0.5f * (a.x - b.x));  // (a - conj b) / (2i)
+            const float2 t = cmul(twr[k], O);
+            *pa = cadd(E, t);
+            const float2 d = csub(E, t);
+            *pb = make_float2(d.x, -d.y);
         }
     }
     __syncthreads();
-    float2 *crow = reinterpret_cast<float2 *>(rows);
     for (int r = threadIdx.x / 64; r < nr; r += FFT_T / 64)
-        for (int k = threadIdx.x & 63; k < M + 2; k += 64) crow[r * (M + 2) + k] = k <= M ? outb[k * ZP + r] : make_float2(0.f, 0.f);  // zsc = M + 2
+        for (int p = threadIdx.x & 63; p < zsc; p += 64) rows[(size_t)r * zsc + p] = p <= M ? tile[p * ZP + r] : make_float2(0.f, 0.f);
 }
 
 // ---- z pass, half-complex -> real (unnormalised: Nz times the inverse), in place ------------------------------
 // E_k = X_k + conj X_{M-k}, O_k = (X_k - conj X_{M-k}) conj(w^k), Z_k = E_k + i O_k (twice the textbook Z: the
-// M-point inverse then yields Nz * x), z = IFFT_M(Z), x_2n = Re z_n, x_2n+1 = Im z_n
+// M-point inverse then yields Nz * x), Z_{M-k} = conj(E_k - i O_k); z = IFFT_M(Z), x_2n = Re z_n, x_2n+1 = Im z_n
 template <int M, int ZRS>
 __global__ void __launch_bounds__(FFT_T) fft_z_c2r_kernel(FftGeom g, float *data, long long nrows)
 {
@@ -568,46 +581,39 @@ __global__ void __launch_bounds__(FFT_T) fft_z_c2r_kernel(FftGeom g, float *data
     extern __shared__ __align__(16) unsigned char fsm[];
     pdl_trigger();  // the constant tables are loaded before pdl_wait(), the data after it
     float2 *tile = reinterpret_cast<float2 *>(fsm);
-    float2 *inb = tile + M * ZP;
-    float2 *tw = inb + max((M + 1) * ZP, ZROWS * g.zsc);
+    float2 *tw = tile + (M + 1) * ZP;
     float2 *twr = tw + M;
-    int *posz = reinterpret_cast<int *>(twr + (M + 1));
-    const int zs = 2 * g.zsc;
+    int *posz = reinterpret_cast<int *>(twr + (M / 2 + 1));
+    const int zsc = g.zsc;
     const long long row0 = (long long)blockIdx.x * ZROWS;
     const int nr = (int)min((long long)ZROWS, nrows - row0);
-    float *rows = data + (size_t)row0 * zs;
+    float2 *rows = reinterpret_cast<float2 *>(data) + (size_t)row0 * zsc;
     load_tw(tw, g.twz, M);
-    load_tw(twr, g.twzr, M + 1);
+    load_tw(twr, g.twzr, M / 2 + 1);
     for (int i = threadIdx.x; i < M; i += FFT_T) posz[i] = g.posz[i];
     pdl_wait();
-    {   // the nr rows are contiguous in memory: 16-byte async copies, row-major [row][zsc]
-        const int nchunk = nr * (zs / 4);
-        for (int i = threadIdx.x; i < nchunk; i += FFT_T) fft_cp_async16(reinterpret_cast<float *>(inb) + 4 * i, rows + 4 * (size_t)i);
-    }
-    fft_cp_async_wait_all();
-    __syncthreads();
-    {
-        const int r = threadIdx.x & (ZROWS - 1);
-        if (r < nr) {
+    for (int r = threadIdx.x / 64; r < nr; r += FFT_T / 64) {
 #pragma unroll 4
-            for (int k = threadIdx.x >> ZRS; k < M; k += FFT_T >> ZRS) {
-                const float2 a = inb[r * (M + 2) + k], b = inb[r * (M + 2) + M - k];
-                const float2 E = make_float2(a.x + b.x, a.y - b.y);
-                const float2 O = cmulc(make_float2(a.x - b.x, a.y + b.y), twr[k]);
-                tile[posz[k] * ZP + r] = make_float2(E.x - O.y, E.y + O.x);  // E + i O
-            }
-        }
+        for (int p = threadIdx.x & 63; p <= M; p += 64) tile[p * ZP + r] = __ldg(rows + (size_t)r * zsc + p);
+    }
+    __syncthreads();
+    for (int w = threadIdx.x; w < (M / 2 + 1) * ZROWS; w += FFT_T) {
+        const int r = w & (ZROWS - 1), k = w >> ZRS;
+        if (r >= nr) continue;
+        float2 *pa = tile + posz[k] * ZP + r;
+        float2 *pb = k == 0 ? tile + M * ZP + r : tile + posz[M - k] * ZP + r;
+        const float2 a = *pa, b = *pb;
+        const float2 E = make_float2(a.x + b.x, a.y - b.y);
+        const float2 O = cmulc(make_float2(a.x - b.x, a.y + b.y), twr[k]);
+        *pa = make_float2(E.x - O.y, E.y + O.x);                        // E + i O
+        if (k != 0 && 2 * k != M) *pb = make_float2(E.x + O.y, O.x - E.y);  // conj(E - i O)
     }
     __syncthreads();
     AxisFFT<M, M, true, ZP, ZRS>::run(tile, nr, tw);
-    if (M <= FFT_T) {
-        constexpr int RPP = FFT_T / M > 0 ? FFT_T / M : 1;
-        const int n = threadIdx.x % M, r0 = threadIdx.x / M;
-#pragma unroll 4
-        for (int r = r0; r < nr; r += RPP) *reinterpret_cast<float2 *>(rows + r * (2 * M + 4) + 2 * n) = tile[n * ZP + r];  // zs = 2 M + 4
-    } else {
-        for (int r = 0; r < nr; r++)
-            for (int n = threadIdx.x; n < M; n += FFT_T) *reinterpret_cast<float2 *>(rows + (size_t)r * zs + 2 * n) = tile[n * ZP + r];
+#pragma unroll 8
+    for (int idx = threadIdx.x; idx < M * ZROWS; idx += FFT_T) {
+        const int n = idx & (M - 1), r = idx / M;
+        if (r < nr) rows[(size_t)r * zsc + n] = tile[n * ZP + r];
     }
 }
 
@@ -667,8 +673,12 @@ void fft_own_axis_order(const pm_ctx *c, int axis, std::vector<int> &freq)
 {
     const int N = c->g.N[axis];
     freq.resize(N);
-    if (!c->own_fft || axis == 2) {
+    if (!c->own_fft) {
         for (int i = 0; i < N; i++) freq[i] = i;
+    } else if (axis == 2) {
+        // half spectrum of the real transform: columns 0 .. N/2 - 1 in the order of the N/2-point stages, column N/2 = Nyquist
+        AxisPlan p = make_axis_plan(N / 2);
+        for (int i = 0; i < N; i++) freq[i] = i < N / 2 ? freq_of_pos(p, i) : i;
     } else {
         AxisPlan p = make_axis_plan(N);
         for (int i = 0; i < N; i++) freq[i] = freq_of_pos(p, i);
@@ -769,11 +779,9 @@ static int fft_z(pm_ctx *c, float *mesh, int nb, bool inverse)
     FftGeom fg = *geom_of(c);
     const int M = g.N[2] / 2;
     long long nrows = (long long)nb * g.N[0] * g.N[1];
-    const int ZRS = M >= 512 ? 3 : 4, ZROWS = 1 << ZRS, ZP = ZROWS + 1;  // fewer rows per CTA for long rows: 3 CTAs per SM
+    const int ZRS = 4, ZROWS = 1 << ZRS, ZP = ZROWS + 1;
     unsigned grid = (unsigned)((nrows + ZROWS - 1) / ZROWS);
-    size_t second = (size_t)(M + 1) * ZP;                       // outb / inb: transposed [M + 1][ZP] or row-major staging
-    if (second < (size_t)ZROWS * (g.zs / 2)) second = (size_t)ZROWS * (g.zs / 2);
-    size_t smem = sizeof(float2) * ((size_t)M * ZP + second + M + (M + 1)) + sizeof(int) * (size_t)M;
+    size_t smem = sizeof(float2) * ((size_t)(M + 1) * ZP + M + (M / 2 + 1)) + sizeof(int) * (size_t)M;
     Timer t(c, inverse ? TC_FFT_Z_C2R : TC_FFT_Z_R2C, 8.0 * (double)g.ng * nb);
 #define Z_CASE(NN, CS_)                                                                                     \
     if (inverse) PM_FFT_LAUNCH(c, "fft_z_c2r_kernel", (fft_z_c2r_kernel<NN, CS_>), grid, smem, fg, mesh, nrows);  \
@@ -785,7 +793,7 @@ static int fft_z(pm_ctx *c, float *mesh, int nb, bool inverse)
         case 64: Z_CASE(64, 4); break;
         case 128: Z_CASE(128, 4); break;
         case 256: Z_CASE(256, 4); break;
-        case 512: Z_CASE(512, 3); break;
+        case 512: Z_CASE(512, 4); break;
         default: return fail(c, PM_EINVAL, "own FFT", "unsupported Nz");
     }
 #undef Z_CASE
