@@ -929,3 +929,95 @@ void orc_ic_vjp(const int N[3], const int L[3], double om, double a0, double amp
     ic_real_of(L, dbar, domega, 1, NULL);
     free(dbar); free(c);
 }
+
+/* ------------------------------------------------------------------------------------ */
+/* 8. Observations between the steps and the cosmological-parameter gradient             */
+/*    (eq. 49 last two lines "O_{i-1}: xi_{i-1} += dJ/dx_{i-1}", L393, L369;     */
+/*    eq. 51 first line, L406, for theta = Omega_m).  SURVEY section 8(f) rows 3 and 4.   */
+/*                                                                                        */
+/*    Objective: J = sum_k w_k J_k, J_k = 1/2 sum_g (delta(x_{i_k}) - target_k)^2, the     */
+/*    mesh objective of section 5 evaluated on the SNAPSHOTS i_k in 0..n (the simplest     */
+/*    observation operator of L179; the light cone of L187 is out of scope).               */
+/*    Loop part of eq. 51 with theta = Omega_m (ICs and objective held fixed):             */
+/*      dJ/dOm = - sum_i [ (pi_i.acc_i d/dOm + zeta_i) K(t_i,t_i,t_{i-1/2})                */
+/*                        + xi_{i-1/2}.p_{i-1/2} dD(t_{i-1/2},t_i,t_{i-1})/dOm            */
+/*                        + (pi_{i-1}.acc_{i-1} d/dOm + zeta_{i-1}) K(t_{i-1},t_{i-1/2},t_{i-1}) ] */
+/*    where "pi.acc d/dOm K" is (pi.acc) dK/dOm, and zeta = pi . d acc/d Om = pi.acc / Om   */
+/*    because acc = F(x) is linear in Om at fixed x (eq. 11).  dK/dOm, dD/dOm: central      */
+/*    differences of the factor functions above (step 1e-4; they are smooth in Om).        */
+/* ------------------------------------------------------------------------------------ */
+static double dot3(long n3, const double *u, const double *v)
+{
+    double t = 0.0;
+    for (long j = 0; j < n3; j++) t += u[j] * v[j];
+    return t;
+}
+
+double orc_run_fwd_adj_obs(const int N[3], const int L[3], double om, int deconv, int n, const double *a,
+                           const double *s0, const double *p0, int n_obs, const int *obs_step, const double *obs_w,
+                           const double *targets, double *s_n, double *p_n, double *xi0, double *pi0, double *J_obs,
+                           double *dJ_dOm)
+{
+    long np = (long)L[0] * L[1] * L[2], n3 = 3 * np;
+    size_t ng = (size_t)N[0] * N[1] * N[2];
+    double *s = (double *)malloc(sizeof(double) * n3), *p = (double *)malloc(sizeof(double) * n3);
+    double *acc = (double *)malloc(sizeof(double) * n3), *x = (double *)malloc(sizeof(double) * n3);
+    double *xi = (double *)calloc(n3, sizeof(double)), *pi = (double *)calloc(n3, sizeof(double));
+    double *alpha = (double *)calloc(n3, sizeof(double)), *g = (double *)malloc(sizeof(double) * n3);
+    double J = 0.0, dth = 0.0;
+    const double h = 1e-4;
+    memcpy(s, s0, sizeof(double) * n3);
+    memcpy(p, p0, sizeof(double) * n3);
+    orc_init_acc(N, L, om, deconv, s, acc);
+    /* forward (eq. 16) with the observations O_i (eq. 17): J_k at the snapshots */
+    for (int i = 0; i <= n; i++) {
+        if (i > 0) orc_step_fwd(N, L, om, deconv, a, i, s, p, acc);
+        for (int k = 0; k < n_obs; k++)
+            if (obs_step[k] == i) {
+                orc_positions(N, L, s, x);
+                double Jk = orc_objective(N, np, x, targets + (size_t)k * ng, NULL);
+                if (J_obs) J_obs[k] = Jk;
+                J += obs_w[k] * Jk;
+            }
+    }
+    if (s_n) memcpy(s_n, s, sizeof(double) * n3);
+    if (p_n) memcpy(p_n, p, sizeof(double) * n3);
+    /* eq. 50: xi_n = dJ/dx_n (zero unless t_n is observed), pi_n = 0, alpha_n = 0 */
+    for (int k = 0; k < n_obs; k++)
+        if (obs_step[k] == n) {
+            orc_positions(N, L, s, x);
+            orc_objective(N, np, x, targets + (size_t)k * ng, g);
+            for (long j = 0; j < n3; j++) xi[j] += obs_w[k] * g[j];
+        }
+    for (int i = n; i >= 1; i--) {
+        double ah = a_half(a, i);
+        double K1 = orc_kick_factor(om, a[i], a[i], ah);                 /* K(t_i, t_i, t_{i-1/2})         */
+        double D = orc_drift_factor(om, ah, a[i], a[i - 1]);             /* D(t_{i-1/2}, t_i, t_{i-1})     */
+        double K2 = orc_kick_factor(om, a[i - 1], ah, a[i - 1]);         /* K(t_{i-1}, t_{i-1/2}, t_{i-1}) */
+        double dK1 = (orc_kick_factor(om + h, a[i], a[i], ah) - orc_kick_factor(om - h, a[i], a[i], ah)) / (2 * h);
+        double dD = (orc_drift_factor(om + h, ah, a[i], a[i - 1]) - orc_drift_factor(om - h, ah, a[i], a[i - 1])) / (2 * h);
+        double dK2 = (orc_kick_factor(om + h, a[i - 1], ah, a[i - 1]) - orc_kick_factor(om - h, a[i - 1], ah, a[i - 1])) / (2 * h);
+        double A = dot3(n3, pi, acc);                                    /* pi_i . acc_i                   */
+        dth -= A * dK1 + (A / om) * K1;
+        for (long j = 0; j < n3; j++) { p[j] += acc[j] * K1; xi[j] -= alpha[j] * K1; }
+        dth -= dot3(n3, xi, p) * dD;                                     /* xi_{i-1/2} . p_{i-1/2}         */
+        for (long j = 0; j < n3; j++) { s[j] += p[j] * D; pi[j] -= xi[j] * D; }
+        force_at(N, L, om, deconv, s, acc);
+        vjp_at(N, L, om, deconv, s, pi, alpha);
+        A = dot3(n3, pi, acc);                                           /* pi_{i-1} . acc_{i-1}           */
+        dth -= A * dK2 + (A / om) * K2;
+        for (long j = 0; j < n3; j++) { p[j] += acc[j] * K2; xi[j] -= alpha[j] * K2; }
+        /* O_{i-1} (eq. 49, last lines): xi_{i-1} += dJ/dx_{i-1}; dJ/dp = 0 for a density objective */
+        for (int k = 0; k < n_obs; k++)
+            if (obs_step[k] == i - 1) {
+                orc_positions(N, L, s, x);
+                orc_objective(N, np, x, targets + (size_t)k * ng, g);
+                for (long j = 0; j < n3; j++) xi[j] += obs_w[k] * g[j];
+            }
+    }
+    if (xi0) memcpy(xi0, xi, sizeof(double) * n3);
+    if (pi0) memcpy(pi0, pi, sizeof(double) * n3);
+    if (dJ_dOm) *dJ_dOm = dth;
+    free(s); free(p); free(acc); free(x); free(xi); free(pi); free(alpha); free(g);
+    return J;
+}

@@ -84,6 +84,8 @@ def lib():
         L.orc_ic.argtypes = [_ip, _ip] + [C.c_double] * 5 + [C.c_int, _dp, _dp, _dp]
         L.orc_ic.restype = C.c_double
         L.orc_ic_vjp.argtypes = [_ip, _ip] + [C.c_double] * 5 + [C.c_int, _dp, _dp, _dp, _dp]
+        L.orc_run_fwd_adj_obs.argtypes = [_ip, _ip, C.c_double, C.c_int, C.c_int, _dp, _dp, _dp, C.c_int, _ip, _dp, _dp] + [_dp] * 6
+        L.orc_run_fwd_adj_obs.restype = C.c_double
         _lib = L
     return _lib
 
@@ -310,4 +312,24 @@ def ic_vjp(N, L, omega_m, a0, amp, omega, xi0, pi0, order=2, ns=-1.5, rc=2.0):
     om = _f64(omega).reshape(-1)
     out = np.zeros_like(om)
     lib().orc_ic_vjp(_i3(N), _i3(L), omega_m, a0, amp, ns, rc, order, _d(om), _d(_f64(xi0)), _d(_f64(pi0)), _d(out))
+    return out
+
+
+# ---- observations between the steps, dJ/dOmega_m (eq. 49 last lines, eq. 51 first line) ----
+def run_fwd_adj_obs(N, L, omega_m, a, s0, p0, obs_steps, obs_weights, targets, deconv=0):
+    """J = sum_k w_k J_k(x_{i_k}); returns s_n, p_n, xi0, pi0, J, J_obs[k], dJ_dOm (loop part of eq. 51)."""
+    a = _f64(a)
+    n = a.shape[0] - 1
+    s0 = _f64(s0)
+    p0 = _f64(p0)
+    steps = np.ascontiguousarray(obs_steps, dtype=np.int32)
+    w = _f64(obs_weights)
+    t = _f64(targets).reshape(len(steps), -1)
+    out = {k: np.zeros_like(s0) for k in ("s_n", "p_n", "xi0", "pi0")}
+    J_obs = np.zeros(len(steps))
+    dth = np.zeros(1)
+    J = lib().orc_run_fwd_adj_obs(_i3(N), _i3(L), omega_m, deconv, n, _d(a), _d(s0), _d(p0), len(steps),
+                                  steps.ctypes.data_as(_ip), _d(w), _d(t), _d(out["s_n"]), _d(out["p_n"]),
+                                  _d(out["xi0"]), _d(out["pi0"]), _d(J_obs), _d(dth))
+    out.update(J=J, J_obs=J_obs, dJ_dOm=float(dth[0]))
     return out

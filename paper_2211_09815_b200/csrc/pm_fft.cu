@@ -19,6 +19,7 @@
 #include <cmath>
 #include <cstdlib>
 #include <cstring>
+#include <type_traits>
 
 #include "pm_internal.cuh"
 
@@ -110,14 +111,21 @@ __device__ __forceinline__ int trow(int pos) { return SWZ ? pos ^ ((pos >> 2) & 
 // ---- one transform along the tile's position axis, everything but the data known at compile time -----------
 // tile [N][PITCH] (float2), columns [0, ncol) of 1 << CS; tw = exp(-2 pi i k / N), k < N (shared memory).
 // Stage of span L, radix R = stage_radix(L): butterfly (blk, j) takes positions blk L + j + m L/R, m < R.
-template <int N, int L, bool INV, int PITCH, int CS>
-__device__ __forceinline__ void fft_stage(float2 *tile, int ncol, const float2 *tw)
+struct NoOut {
+    __device__ __forceinline__ void operator()(int, int, float2) const {}
+};
+// OUT = NoOut: the stage works in place on the tile.  Any other OUT receives the results instead -- out(position, column,
+// value) -- so that the LAST stage of a transform can hand them straight to global memory (no store to the tile, no
+// barrier, no copy-out pass).
+template <int N, int L, bool INV, int PITCH, int CS, class OUT>
+__device__ __forceinline__ void fft_stage_impl(float2 *tile, int ncol, const float2 *tw, const OUT &out)
 {
     constexpr int R = stage_radix(L);
     constexpr int Lr = L / R, twstep = N / L;
     constexpr int nwork = (N / R) << CS;
     constexpr bool SWZ = CS == 3 && PITCH == 8;      // rows of 8 unpadded columns: see trow()
     constexpr bool SAME = !SWZ || Lr % 8 == 0;        // every element of a butterfly gets the same row swizzle
+    constexpr bool TO_TILE = std::is_same<OUT, NoOut>::value;
 #pragma unroll 1
     for (int wk = threadIdx.x; wk < nwork; wk += FFT_T) {
         const int col = wk & ((1 << CS) - 1);
@@ -139,10 +147,16 @@ __device__ __forceinline__ void fft_stage(float2 *tile, int ncol, const float2 *
             const int q = bitrev(i, R);
             float2 o = v[i];
             if (!INV && Lr > 1 && q != 0) o = cmul(o, tw[j * q * twstep]);
-            if (SAME) p[q * Lr * PITCH] = o;
+            if (!TO_TILE) out(base + q * Lr, col, o);
+            else if (SAME) p[q * Lr * PITCH] = o;
             else tile[trow<SWZ>(base + q * Lr) * PITCH + col] = o;
         }
     }
+}
+template <int N, int L, bool INV, int PITCH, int CS>
+__device__ __forceinline__ void fft_stage(float2 *tile, int ncol, const float2 *tw)
+{
+    fft_stage_impl<N, L, INV, PITCH, CS, NoOut>(tile, ncol, tw, NoOut());
 }
 
 template <int N, int L, bool INV, int PITCH, int CS>
@@ -225,6 +239,42 @@ __device__ __forceinline__ void load_tw(float2 *dst, const float2 *src, int n)
 
 // ---- y pass: in-place transform along y of nb meshes ---------------------------------------------------------
 // grid = (column tiles along z, Nx, nb); dynamic shared memory: tile [Ny][1 << CS] + Ny twiddles
+__host__ __device__ constexpr int last_span(int N)
+{
+    int L = N;
+    while (stage_radix(L) != L) L /= stage_radix(L);
+    return L;
+}
+
+// the stages with span > LSTOP only (forward: descending spans, inverse: ascending); every stage is followed by a barrier
+template <int N, int L, bool INV, int PITCH, int CS, int LSTOP>
+struct AxisFFTPartial {
+    static constexpr int R = stage_radix(L);
+    static __device__ __forceinline__ void run(float2 *tile, int ncol, const float2 *tw)
+    {
+        if (!INV) {
+            fft_stage<N, L, false, PITCH, CS>(tile, ncol, tw);
+            __syncthreads();
+            AxisFFTPartial<N, L / R, INV, PITCH, CS, LSTOP>::run(tile, ncol, tw);
+        } else {
+            AxisFFTPartial<N, L / R, INV, PITCH, CS, LSTOP>::run(tile, ncol, tw);
+            fft_stage<N, L, true, PITCH, CS>(tile, ncol, tw);
+            __syncthreads();
+        }
+    }
+};
+template <int N, int LS, bool INV, int PITCH, int CS>
+struct AxisFFTPartial<N, LS, INV, PITCH, CS, LS> {
+    static __device__ __forceinline__ void run(float2 *, int, const float2 *) {}
+};
+
+// result (position, column) -> base[position * stride + column]
+struct StoreOut {
+    float2 *base;
+    long long stride;
+    __device__ __forceinline__ void operator()(int pos, int col, float2 v) const { base[(size_t)pos * stride + col] = v; }
+};
+
 template <int NY, int CS, bool INV>
 __global__ void __launch_bounds__(FFT_T) fft_y_kernel(FftGeom g, float2 *data)
 {
@@ -240,8 +290,16 @@ __global__ void __launch_bounds__(FFT_T) fft_y_kernel(FftGeom g, float2 *data)
     tile_load<NY, CS>(tile, base, g.zsc, ncol);
     fft_cp_async_wait_all();
     __syncthreads();
-    AxisFFT<NY, NY, INV, B, CS>::run(tile, ncol, tw);
-    tile_store<NY, CS>(tile, base, g.zsc, ncol);
+    // the last stage writes its results straight to global memory (the CTA has read all of its columns by now)
+    const StoreOut out = {base, g.zsc};
+    if (!INV) {
+        constexpr int RL = last_span(NY);
+        AxisFFTPartial<NY, NY, false, B, CS, RL>::run(tile, ncol, tw);
+        fft_stage_impl<NY, RL, false, B, CS>(tile, ncol, tw, out);
+    } else {
+        AxisFFTPartial<NY, NY / stage_radix(NY), true, B, CS, 1>::run(tile, ncol, tw);
+        fft_stage_impl<NY, NY, true, B, CS>(tile, ncol, tw, out);
+    }
 }
 
 // G(k) = c0 dec / k^2 of one mode, fp64 rounded to fp32 once; G(0) = 0 (R9).  The x-dependent table entries come from
@@ -275,35 +333,6 @@ __device__ __forceinline__ float mode_green(const GreenCol &c, double k2x, doubl
 // memory, and the two back-transforms of the force kernel (f_x, and the common part of f_y, f_z) run one after the other
 // through the same tile.  Half the shared memory of a two-tile design: 8 columns (64-byte pieces) at Nx = 1024 with two
 // CTAs per SM, four CTAs per SM at 512.
-__host__ __device__ constexpr int last_span(int N)
-{
-    int L = N;
-    while (stage_radix(L) != L) L /= stage_radix(L);
-    return L;
-}
-
-// the stages with span > LSTOP only (forward: descending spans, inverse: ascending); every stage is followed by a barrier
-template <int N, int L, bool INV, int PITCH, int CS, int LSTOP>
-struct AxisFFTPartial {
-    static constexpr int R = stage_radix(L);
-    static __device__ __forceinline__ void run(float2 *tile, int ncol, const float2 *tw)
-    {
-        if (!INV) {
-            fft_stage<N, L, false, PITCH, CS>(tile, ncol, tw);
-            __syncthreads();
-            AxisFFTPartial<N, L / R, INV, PITCH, CS, LSTOP>::run(tile, ncol, tw);
-        } else {
-            AxisFFTPartial<N, L / R, INV, PITCH, CS, LSTOP>::run(tile, ncol, tw);
-            fft_stage<N, L, true, PITCH, CS>(tile, ncol, tw);
-            __syncthreads();
-        }
-    }
-};
-template <int N, int LS, bool INV, int PITCH, int CS>
-struct AxisFFTPartial<N, LS, INV, PITCH, CS, LS> {
-    static __device__ __forceinline__ void run(float2 *, int, const float2 *) {}
-};
-
 template <int NX, int CS>
 struct XPlan {
     static constexpr int B = 1 << CS;
@@ -329,15 +358,43 @@ struct XPlan {
         for (int m = 0; m < RL; m++) x[m] = v[bitrev(m, RL)];
     }
     // first inverse stage: takes the RL spectrum elements, leaves its outputs in the tile for the remaining stages
-    static __device__ __forceinline__ void first_inv(float2 *tile, int col, int pos0, float2 (&v)[RL])
+    // (when the whole transform is this one stage, NX == RL, the outputs are final and go to `out` instead)
+    template <class OUT>
+    static __device__ __forceinline__ void first_inv(float2 *tile, int col, int pos0, float2 (&v)[RL], const OUT &out)
     {
         reg_dft<RL, true>(v);
 #pragma unroll
-        for (int i = 0; i < RL; i++) tile[(trow<CS == 3>(pos0 + bitrev(i, RL)) << CS) + col] = v[i];
+        for (int i = 0; i < RL; i++) {
+            if (NX == RL) out(pos0 + bitrev(i, RL), col, v[i]);
+            else tile[(trow<CS == 3>(pos0 + bitrev(i, RL)) << CS) + col] = v[i];
+        }
+    }
+    // the inverse stages after the first one; the last of them hands its results to `out`
+    template <class OUT>
+    static __device__ __forceinline__ void inv_rest(float2 *tile, int ncol, const float2 *tw, const OUT &out)
+    {
+        if (NX != RL) {
+            __syncthreads();
+            AxisFFTPartial<NX, NX / stage_radix(NX), true, B, CS, (NX != RL ? RL : 1)>::run(tile, ncol, tw);
+            fft_stage_impl<NX, NX, true, B, CS>(tile, ncol, tw, out);
+        }
     }
 };
 
 #define PM_X_MINBLOCKS(NX) ((NX) >= 1024 ? 2 : ((NX) >= 512 ? 3 : 2))
+
+// T(position, column) -> f_y = i kt_y T and f_z = i kt_z T (kt_z of the thread's own column: a thread only ever sees one)
+struct StoreYZ {
+    float2 *fy;
+    long long stride, cstride;
+    float kty, ktz;
+    __device__ __forceinline__ void operator()(int pos, int col, float2 t) const
+    {
+        float2 *dst = fy + (size_t)pos * stride + col;
+        dst[0] = make_float2(-kty * t.y, kty * t.x);
+        dst[cstride] = make_float2(-ktz * t.y, ktz * t.x);
+    }
+};
 
 // ---- x pass fused with the force operator: rho(k) -> f_d(k) = i kt_d G rho(k), d = 1..3, back-transformed along x ----
 // grid = (column tiles along z, Ny); shared: one tile + Nx twiddles + the x-dependent k tables
@@ -385,6 +442,8 @@ __global__ void __launch_bounds__(FFT_T, PM_X_MINBLOCKS(NX)) fft_x_force_kernel(
             }
         }
     }
+    const StoreOut out_x = {f + off, stride};
+    const StoreYZ out_yz = {f + g.cstride + off, stride, g.cstride, kty, (float)g.ktab[6 * g.tabn + min(col0 + (int)(threadIdx.x & (B - 1)), g.N[2] / 2)]};
     // f_x: back-transform of i kt_x h (a thread rewrites only the tile elements it has just read: no barrier before)
 #pragma unroll
     for (int it = 0; it < IT; it++) {
@@ -396,36 +455,18 @@ __global__ void __launch_bounds__(FFT_T, PM_X_MINBLOCKS(NX)) fft_x_force_kernel(
             const float c = ktx[pos0 + m];
             v[m] = make_float2(-c * h[it][m].y, c * h[it][m].x);
         }
-        P::first_inv(tile, col, pos0, v);
+        P::first_inv(tile, col, pos0, v, out_x);
     }
-    __syncthreads();
-    AxisFFTPartial<NX, NX, true, B, CS, RL>::run(tile, ncol, tw);
-    tile_store<NX, CS>(tile, f + off, stride, ncol);
+    P::inv_rest(tile, ncol, tw, out_x);   // the last stage stores f_x
     __syncthreads();
     // kt_y and kt_z do not depend on x, so ONE back-transform T of h serves f_y = i kt_y T and f_z = i kt_z T
 #pragma unroll
     for (int it = 0; it < IT; it++) {
         int col, pos0;
         if (!P::item(it, ncol, col, pos0)) continue;
-        P::first_inv(tile, col, pos0, h[it]);
+        P::first_inv(tile, col, pos0, h[it], out_yz);
     }
-    __syncthreads();
-    AxisFFTPartial<NX, NX, true, B, CS, RL>::run(tile, ncol, tw);
-    {
-        constexpr int HB = 1 << (CS - 1);  // 16-byte stores of column pairs
-        const int cp = threadIdx.x & (HB - 1);
-        if (2 * cp < ncol) {
-            const float kz0 = (float)g.ktab[6 * g.tabn + min(col0 + 2 * cp, g.N[2] / 2)];
-            const float kz1 = (float)g.ktab[6 * g.tabn + min(col0 + 2 * cp + 1, g.N[2] / 2)];
-#pragma unroll 4
-            for (int pos = threadIdx.x >> (CS - 1); pos < NX; pos += FFT_T >> (CS - 1)) {
-                const float4 t4 = *reinterpret_cast<const float4 *>(tile + (trow<CS == 3>(pos) << CS) + 2 * cp);
-                float2 *dst = f + g.cstride + off + (size_t)pos * stride + 2 * cp;
-                *reinterpret_cast<float4 *>(dst) = make_float4(-kty * t4.y, kty * t4.x, -kty * t4.w, kty * t4.z);
-                *reinterpret_cast<float4 *>(dst + g.cstride) = make_float4(-kz0 * t4.y, kz0 * t4.x, -kz1 * t4.w, kz1 * t4.z);
-            }
-        }
-    }
+    P::inv_rest(tile, ncol, tw, out_yz);  // the last stage stores f_y and f_z
 }
 
 // ---- x pass fused with the adjoint operator: psi(k) = -i G sum_d kt_d Pi_d(k), back-transformed along x ----------
@@ -485,6 +526,7 @@ __global__ void __launch_bounds__(FFT_T, PM_X_MINBLOCKS(NX)) fft_x_adjoint_kerne
     }
     __syncthreads();
     AxisFFTPartial<NX, NX, false, B, CS, RL>::run(tile, ncol, tw);
+    const StoreOut out_psi = {psi + off, stride};
     {
         const int colt = threadIdx.x & (B - 1);
         const GreenCol gc = green_col(g, iy, min(col0 + colt, g.N[2] / 2));
@@ -502,120 +544,130 @@ __global__ void __launch_bounds__(FFT_T, PM_X_MINBLOCKS(NX)) fft_x_adjoint_kerne
                 // times -i G: (re, im) -> (G im, -G re)
                 a[m] = make_float2(G * (c * v.y + a[m].y), -G * (c * v.x + a[m].x));
             }
-            P::first_inv(tile, col, pos0, a);
+            P::first_inv(tile, col, pos0, a, out_psi);
         }
     }
-    __syncthreads();
-    AxisFFTPartial<NX, NX, true, B, CS, RL>::run(tile, ncol, tw);
-    tile_store<NX, CS>(tile, psi + off, stride, ncol);
+    P::inv_rest(tile, ncol, tw, out_psi);  // the last stage stores psi
 }
 
-// ---- z pass, real -> half-complex, in place on ZROWS consecutive z-rows per CTA, ONE tile ---------------------------
+// ---- z pass, real -> half-complex, in place on ZROWS consecutive z-rows per CTA ---------------------------------
 // row = [zs floats] -> [zsc complex]; x_n real, n < Nz = 2M: z_n = x_2n + i x_2n+1, Z = FFT_M(z),
-// E_k = (Z_k + conj Z_{M-k}) / 2, O_k = (Z_k - conj Z_{M-k}) / (2i), X_k = E_k + w^k O_k, w = e^{-2 pi i / Nz}, k = 0..M,
-// and X_{M-k} = conj(E_k - w^k O_k): one thread turns the pair (Z_k, Z_{M-k}) into (X_k, X_{M-k}) IN PLACE.
-// The rows go straight from global memory into the transposed tile [position][row] and back (a warp moves 32 consecutive
-// elements of one row: coalesced; the odd tile pitch keeps the strided shared-memory side free of bank conflicts), so
-// there is neither a staging buffer nor a second tile.  The spectrum is left in the tile's own order: column p < M of a
-// row holds the frequency the forward stages leave at position p (digit-reversed, as along x and y), column M the Nyquist
-// frequency; only the k tables know (R26).
-// shared: tile [M + 1][ZP] + M twiddles + (M/2 + 1) post twiddles + M positions
+// E_k = (Z_k + conj Z_{M-k}) / 2, O_k = (Z_k - conj Z_{M-k}) / (2i), X_k = E_k + w^k O_k, w = e^{-2 pi i / Nz}, k = 0..M
+// shared: tile [M][ZP] + out [M + 1][ZP] + M twiddles + (M + 1) post twiddles + M positions
 template <int M, int ZRS>
 __global__ void __launch_bounds__(FFT_T) fft_z_r2c_kernel(FftGeom g, float *data, long long nrows)
 {
-    constexpr int ZROWS = 1 << ZRS, ZP = ZROWS + 1;  // z-rows per CTA; tile pitch
+    constexpr int ZROWS = 1 << ZRS, ZP = ZROWS + 1;  // z-rows per CTA; padded pitch of the transposing buffer
+    constexpr int TP = ZRS == 3 ? 8 : ZP;            // tile pitch: 8 rows are kept unpadded and swizzled instead (trow)
+#define ZT(pos) (trow<ZRS == 3>(pos) * TP)
     extern __shared__ __align__(16) unsigned char fsm[];
     pdl_trigger();  // the constant tables are loaded before pdl_wait(), the data after it
     float2 *tile = reinterpret_cast<float2 *>(fsm);
-    float2 *tw = tile + (M + 1) * ZP;
+    float2 *outb = tile + M * TP;
+    float2 *tw = outb + max((M + 1) * ZP, ZROWS * g.zsc);
     float2 *twr = tw + M;
-    int *posz = reinterpret_cast<int *>(twr + (M / 2 + 1));
-    const int zsc = g.zsc;
+    int *posz = reinterpret_cast<int *>(twr + (M + 1));
+    const int zs = 2 * g.zsc;
     const long long row0 = (long long)blockIdx.x * ZROWS;
     const int nr = (int)min((long long)ZROWS, nrows - row0);
-    float2 *rows = reinterpret_cast<float2 *>(data) + (size_t)row0 * zsc;
+    float *rows = data + (size_t)row0 * zs;
+    // the nr rows are contiguous in memory: 16-byte async copies into a row-major staging area (which shares its
+    // shared memory with outb), then the transposing fill of the tile
+    float *stage = reinterpret_cast<float *>(outb);
     load_tw(tw, g.twz, M);
-    load_tw(twr, g.twzr, M / 2 + 1);
+    load_tw(twr, g.twzr, M + 1);
     for (int i = threadIdx.x; i < M; i += FFT_T) posz[i] = g.posz[i];
     pdl_wait();
-#pragma unroll 8
-    for (int idx = threadIdx.x; idx < M * ZROWS; idx += FFT_T) {
-        const int n = idx & (M - 1), r = idx / M;
-        if (r < nr) tile[n * ZP + r] = __ldg(rows + (size_t)r * zsc + n);
+    {
+        const int nchunk = nr * (zs / 4);
+        for (int i = threadIdx.x; i < nchunk; i += FFT_T) fft_cp_async16(stage + 4 * i, rows + 4 * (size_t)i);
     }
+    fft_cp_async_wait_all();
     __syncthreads();
-    AxisFFT<M, M, false, ZP, ZRS>::run(tile, nr, tw);
-    for (int w = threadIdx.x; w < (M / 2 + 1) * ZROWS; w += FFT_T) {
-        const int r = w & (ZROWS - 1), k = w >> ZRS;
-        if (r >= nr) continue;
-        float2 *pa = tile + posz[k] * ZP + r;
-        const float2 a = *pa;
-        if (k == 0) {
-            *pa = make_float2(a.x + a.y, 0.f);
-            tile[M * ZP + r] = make_float2(a.x - a.y, 0.f);
-        } else if (2 * k == M) {
-            *pa = make_float2(a.x, -a.y);
-        } else {
-            float2 *pb = tile + posz[M - k] * ZP + r;
-            const float2 b = *pb;
-            const float2 E = make_float2(0.5f * (a.x + b.x), 0.5f * (a.y - b.y));
-            const float2 O = make_float2(0.5f * (a.y + b.y), -0.5f * (a.x - b.x));  // (a - conj b) / (2i)
-            const float2 t = cmul(twr[k], O);
-            *pa = cadd(E, t);
-            const float2 d = csub(E, t);
-            *pb = make_float2(d.x, -d.y);
+    {
+        const int r = threadIdx.x & (ZROWS - 1);
+        if (r < nr) {
+#pragma unroll 4
+            for (int n = threadIdx.x >> ZRS; n < M; n += FFT_T >> ZRS) tile[ZT(n) + r] = *reinterpret_cast<const float2 *>(stage + r * (2 * M + 4) + 2 * n);
         }
     }
     __syncthreads();
+    AxisFFT<M, M, false, TP, ZRS>::run(tile, nr, tw);
+
+    {
+        const int r = threadIdx.x & (ZROWS - 1);
+        if (r < nr) {
+#pragma unroll 4
+            for (int k = threadIdx.x >> ZRS; k <= M; k += FFT_T >> ZRS) {
+                const int km = k == M ? 0 : k, kc = (k == 0 || k == M) ? 0 : M - k;
+                const float2 a = tile[ZT(posz[km]) + r], b = tile[ZT(posz[kc]) + r];
+                const float2 E = make_float2(0.5f * (a.x + b.x), 0.5f * (a.y - b.y));
+                const float2 O = make_float2(0.5f * (a.y + b.y), -0.5f * (a.x - b.x));  // (a - conj b) / (2i)
+                outb[k * ZP + r] = cadd(E, cmul(twr[k], O));
+            }
+        }
+    }
+    __syncthreads();
+    float2 *crow = reinterpret_cast<float2 *>(rows);
     for (int r = threadIdx.x / 64; r < nr; r += FFT_T / 64)
-        for (int p = threadIdx.x & 63; p < zsc; p += 64) rows[(size_t)r * zsc + p] = p <= M ? tile[p * ZP + r] : make_float2(0.f, 0.f);
+        for (int k = threadIdx.x & 63; k < M + 2; k += 64) crow[r * (M + 2) + k] = k <= M ? outb[k * ZP + r] : make_float2(0.f, 0.f);  // zsc = M + 2
 }
 
 // ---- z pass, half-complex -> real (unnormalised: Nz times the inverse), in place ------------------------------
 // E_k = X_k + conj X_{M-k}, O_k = (X_k - conj X_{M-k}) conj(w^k), Z_k = E_k + i O_k (twice the textbook Z: the
-// M-point inverse then yields Nz * x), Z_{M-k} = conj(E_k - i O_k); z = IFFT_M(Z), x_2n = Re z_n, x_2n+1 = Im z_n
+// M-point inverse then yields Nz * x), z = IFFT_M(Z), x_2n = Re z_n, x_2n+1 = Im z_n
 template <int M, int ZRS>
 __global__ void __launch_bounds__(FFT_T) fft_z_c2r_kernel(FftGeom g, float *data, long long nrows)
 {
-    constexpr int ZROWS = 1 << ZRS, ZP = ZROWS + 1;  // z-rows per CTA; tile pitch
+    constexpr int ZROWS = 1 << ZRS, ZP = ZROWS + 1;  // z-rows per CTA; padded pitch of the transposing buffer
+    constexpr int TP = ZRS == 3 ? 8 : ZP;            // tile pitch: 8 rows are kept unpadded and swizzled instead (trow)
+#define ZT(pos) (trow<ZRS == 3>(pos) * TP)
     extern __shared__ __align__(16) unsigned char fsm[];
     pdl_trigger();  // the constant tables are loaded before pdl_wait(), the data after it
     float2 *tile = reinterpret_cast<float2 *>(fsm);
-    float2 *tw = tile + (M + 1) * ZP;
+    float2 *inb = tile + M * TP;
+    float2 *tw = inb + max((M + 1) * ZP, ZROWS * g.zsc);
     float2 *twr = tw + M;
-    int *posz = reinterpret_cast<int *>(twr + (M / 2 + 1));
-    const int zsc = g.zsc;
+    int *posz = reinterpret_cast<int *>(twr + (M + 1));
+    const int zs = 2 * g.zsc;
     const long long row0 = (long long)blockIdx.x * ZROWS;
     const int nr = (int)min((long long)ZROWS, nrows - row0);
-    float2 *rows = reinterpret_cast<float2 *>(data) + (size_t)row0 * zsc;
+    float *rows = data + (size_t)row0 * zs;
     load_tw(tw, g.twz, M);
-    load_tw(twr, g.twzr, M / 2 + 1);
+    load_tw(twr, g.twzr, M + 1);
     for (int i = threadIdx.x; i < M; i += FFT_T) posz[i] = g.posz[i];
     pdl_wait();
-    for (int r = threadIdx.x / 64; r < nr; r += FFT_T / 64) {
+    {   // the nr rows are contiguous in memory: 16-byte async copies, row-major [row][zsc]
+        const int nchunk = nr * (zs / 4);
+        for (int i = threadIdx.x; i < nchunk; i += FFT_T) fft_cp_async16(reinterpret_cast<float *>(inb) + 4 * i, rows + 4 * (size_t)i);
+    }
+    fft_cp_async_wait_all();
+    __syncthreads();
+    {
+        const int r = threadIdx.x & (ZROWS - 1);
+        if (r < nr) {
 #pragma unroll 4
-        for (int p = threadIdx.x & 63; p <= M; p += 64) tile[p * ZP + r] = __ldg(rows + (size_t)r * zsc + p);
+            for (int k = threadIdx.x >> ZRS; k < M; k += FFT_T >> ZRS) {
+                const float2 a = inb[r * (M + 2) + k], b = inb[r * (M + 2) + M - k];
+                const float2 E = make_float2(a.x + b.x, a.y - b.y);
+                const float2 O = cmulc(make_float2(a.x - b.x, a.y + b.y), twr[k]);
+                tile[ZT(posz[k]) + r] = make_float2(E.x - O.y, E.y + O.x);  // E + i O
+            }
+        }
     }
     __syncthreads();
-    for (int w = threadIdx.x; w < (M / 2 + 1) * ZROWS; w += FFT_T) {
-        const int r = w & (ZROWS - 1), k = w >> ZRS;
-        if (r >= nr) continue;
-        float2 *pa = tile + posz[k] * ZP + r;
-        float2 *pb = k == 0 ? tile + M * ZP + r : tile + posz[M - k] * ZP + r;
-        const float2 a = *pa, b = *pb;
-        const float2 E = make_float2(a.x + b.x, a.y - b.y);
-        const float2 O = cmulc(make_float2(a.x - b.x, a.y + b.y), twr[k]);
-        *pa = make_float2(E.x - O.y, E.y + O.x);                        // E + i O
-        if (k != 0 && 2 * k != M) *pb = make_float2(E.x + O.y, O.x - E.y);  // conj(E - i O)
-    }
-    __syncthreads();
-    AxisFFT<M, M, true, ZP, ZRS>::run(tile, nr, tw);
-#pragma unroll 8
-    for (int idx = threadIdx.x; idx < M * ZROWS; idx += FFT_T) {
-        const int n = idx & (M - 1), r = idx / M;
-        if (r < nr) rows[(size_t)r * zsc + n] = tile[n * ZP + r];
+    AxisFFT<M, M, true, TP, ZRS>::run(tile, nr, tw);
+    if (M <= FFT_T) {
+        constexpr int RPP = FFT_T / M > 0 ? FFT_T / M : 1;
+        const int n = threadIdx.x % M, r0 = threadIdx.x / M;
+#pragma unroll 4
+        for (int r = r0; r < nr; r += RPP) *reinterpret_cast<float2 *>(rows + r * (2 * M + 4) + 2 * n) = tile[ZT(n) + r];  // zs = 2 M + 4
+    } else {
+        for (int r = 0; r < nr; r++)
+            for (int n = threadIdx.x; n < M; n += FFT_T) *reinterpret_cast<float2 *>(rows + (size_t)r * zs + 2 * n) = tile[ZT(n) + r];
     }
 }
+#undef ZT
 
 // ---- host ------------------------------------------------------------------------------------------------------
 static bool is_pow2(int v) { return v > 0 && (v & (v - 1)) == 0; }
@@ -673,12 +725,8 @@ void fft_own_axis_order(const pm_ctx *c, int axis, std::vector<int> &freq)
 {
     const int N = c->g.N[axis];
     freq.resize(N);
-    if (!c->own_fft) {
+    if (!c->own_fft || axis == 2) {
         for (int i = 0; i < N; i++) freq[i] = i;
-    } else if (axis == 2) {
-        // half spectrum of the real transform: columns 0 .. N/2 - 1 in the order of the N/2-point stages, column N/2 = Nyquist
-        AxisPlan p = make_axis_plan(N / 2);
-        for (int i = 0; i < N; i++) freq[i] = i < N / 2 ? freq_of_pos(p, i) : i;
     } else {
         AxisPlan p = make_axis_plan(N);
         for (int i = 0; i < N; i++) freq[i] = freq_of_pos(p, i);
@@ -779,9 +827,12 @@ static int fft_z(pm_ctx *c, float *mesh, int nb, bool inverse)
     FftGeom fg = *geom_of(c);
     const int M = g.N[2] / 2;
     long long nrows = (long long)nb * g.N[0] * g.N[1];
-    const int ZRS = 4, ZROWS = 1 << ZRS, ZP = ZROWS + 1;
+    const int ZRS = M >= 512 ? 3 : 4, ZROWS = 1 << ZRS, ZP = ZROWS + 1;  // fewer rows per CTA for long rows: 3 CTAs per SM
     unsigned grid = (unsigned)((nrows + ZROWS - 1) / ZROWS);
-    size_t smem = sizeof(float2) * ((size_t)(M + 1) * ZP + M + (M / 2 + 1)) + sizeof(int) * (size_t)M;
+    size_t second = (size_t)(M + 1) * ZP;                       // outb / inb: transposed [M + 1][ZP] or row-major staging
+    if (second < (size_t)ZROWS * (g.zs / 2)) second = (size_t)ZROWS * (g.zs / 2);
+    const int TP = ZRS == 3 ? 8 : ZP;                           // tile pitch (8 unpadded, swizzled rows: see trow)
+    size_t smem = sizeof(float2) * ((size_t)M * TP + second + M + (M + 1)) + sizeof(int) * (size_t)M;
     Timer t(c, inverse ? TC_FFT_Z_C2R : TC_FFT_Z_R2C, 8.0 * (double)g.ng * nb);
 #define Z_CASE(NN, CS_)                                                                                     \
     if (inverse) PM_FFT_LAUNCH(c, "fft_z_c2r_kernel", (fft_z_c2r_kernel<NN, CS_>), grid, smem, fg, mesh, nrows);  \
@@ -793,7 +844,7 @@ static int fft_z(pm_ctx *c, float *mesh, int nb, bool inverse)
         case 64: Z_CASE(64, 4); break;
         case 128: Z_CASE(128, 4); break;
         case 256: Z_CASE(256, 4); break;
-        case 512: Z_CASE(512, 4); break;
+        case 512: Z_CASE(512, 3); break;
         default: return fail(c, PM_EINVAL, "own FFT", "unsupported Nz");
     }
 #undef Z_CASE
