@@ -155,6 +155,20 @@ int pm_run_fwd_adj_host(pm_ctx *ctx, const float *host_s0, const float *host_p0,
                         const float *host_delta_target, float *host_s_n, float *host_p_n, double *host_J,
                         float *host_xi0, float *host_pi0, float *host_dJ_ds0, float *host_s_rec, float *host_p_rec);
 
+/* ---- observations between the steps and the cosmological-parameter gradient (eq. 49 last lines L393; eq. 51) ----
+ * J = sum_k w_k J_k, J_k = 1/2 sum_g (delta(x_{i_k}) - target_k)^2 on the snapshots i_k in 0..n (host_obs_step, any order,
+ * n_obs <= PM_MAX_OBS; dev_targets[n_obs][Nx][Ny][Nz]): the observation operator O_{i-1} of eq. 49 adds w_k dJ_k/dx to
+ * xi_{i-1} between adjoint steps.  host_J = J, host_J_obs[k] = J_k (may be NULL).  host_dJ_dOm (may be NULL): the loop
+ * part of eq. 51's first line for theta = Omega_m at fixed (s0, p0) -- sum over the steps of
+ * (pi.acc d/dOm + zeta) K + xi.p dD/dOm with zeta = pi . d acc/d Om = pi.acc / Om (eq. 11 is linear in Om) and the
+ * factor derivatives by central differences on the host; requesting it runs the adjoint steps unchained.
+ * Other arguments and the single final synchronisation as pm_run_fwd_adj. */
+enum { PM_MAX_OBS = 64 };
+int pm_run_fwd_adj_obs(pm_ctx *ctx, const float *dev_s0, const float *dev_p0, int n_obs, const int32_t *host_obs_step,
+                       const double *host_obs_w, const float *dev_targets, float *dev_s_n, float *dev_p_n,
+                       double *host_J, double *host_J_obs, float *dev_xi0, float *dev_pi0, float *dev_dJ_ds0,
+                       double *host_dJ_dOm);
+
 /* ---- initial conditions from white noise, and dJ/d(omega) (eq. 2-6; eq. 51 second line L406) ----------------
  * dev_omega[Lx][Ly][Lz]: real white noise on the particle lattice (L89).  delta_1(k) = amp sqrt(P(k)) omega(k) with
  * P(k) = k^ns exp(-(rc k)^2), k in radians per mesh cell (eq. 6; the volume factor is part of amp; the configs' recipe is

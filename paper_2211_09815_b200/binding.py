@@ -55,6 +55,8 @@ _SIGS = {
     "pm_host_ic_factors": (_int, [_dbl, _dbl, C.POINTER(_dbl)]),
     "pm_ic_fwd": (_int, [_vp, _vp, _dbl, _dbl, _dbl, _int, _vp, _vp]),
     "pm_ic_vjp": (_int, [_vp, _vp, _dbl, _dbl, _dbl, _int, _vp, _vp, _vp]),
+    "pm_run_fwd_adj_obs": (_int, [_vp, _vp, _vp, _int, C.POINTER(C.c_int32), C.POINTER(_dbl), _vp, _vp, _vp,
+                                  C.POINTER(_dbl), C.POINTER(_dbl), _vp, _vp, _vp, C.POINTER(_dbl)]),
     "pm_scatter": (_int, [_vp, _i64, _vp, _vp, _int, _vp]),
     "pm_gather": (_int, [_vp, _i64, _vp, _vp, _int, _vp]),
     "pm_gather_grad": (_int, [_vp, _i64, _vp, _vp, _int, _vp, _vp]),
@@ -249,6 +251,21 @@ class PM:
         alpha = self._new(x.shape[0], 3)
         self._call(_lib.pm_force_vjp, x.shape[0], _ptr(x, "x"), _ptr(pi, "pi"), acc.data_ptr(), alpha.data_ptr())
         return acc, alpha
+
+    def run_fwd_adj_obs(self, s0, p0, obs_steps, obs_weights, targets, want_dJ_dOm=False):
+        """forward + adjoint run with the mesh objective on several snapshots (eq. 49's O operator) and, optionally,
+        the loop part of dJ/dOmega_m (eq. 51).  targets: [n_obs, Nx, Ny, Nz] device tensor."""
+        k = len(obs_steps)
+        steps = (C.c_int32 * k)(*[int(v) for v in obs_steps])
+        w = (_dbl * k)(*[float(v) for v in obs_weights])
+        out = {n: self._new(self.np, 3) for n in ("s_n", "p_n", "xi0", "pi0", "dJ_ds0")}
+        J, Jk, dth = _dbl(0.0), (_dbl * k)(), _dbl(0.0)
+        self._check(_lib.pm_run_fwd_adj_obs(self._h, _ptr(s0, "s0"), _ptr(p0, "p0"), k, steps, w, _ptr(targets, "targets"),
+                                            out["s_n"].data_ptr(), out["p_n"].data_ptr(), C.byref(J), Jk,
+                                            out["xi0"].data_ptr(), out["pi0"].data_ptr(), out["dJ_ds0"].data_ptr(),
+                                            C.byref(dth) if want_dJ_dOm else None), "pm_run_fwd_adj_obs")
+        out.update(J=J.value, J_obs=list(Jk), dJ_dOm=dth.value if want_dJ_dOm else None)
+        return out
 
     # ---- initial conditions (eq. 2-6) and dJ/d(omega) (eq. 51) ----
     def ic_fwd(self, omega, amp, order=2, ns=-1.5, rc=2.0):

@@ -707,11 +707,9 @@ bool fft_own_supported(const Geometry &g)
 {
     const char *e = getenv("PM_FFT");
     if (e && strcmp(e, "cufft") == 0) return false;
-    // above 512 the x pass strides over more 2 MB pages than the TLBs like and cuFFT's passes are as fast
-    // (measured at 1024^3, profiles/); PM_FFT=own forces the own passes there too
-    const bool force = e && strcmp(e, "own") == 0;
+    // powers of two from 16 to 1024 per axis (at 1024^3 the own passes take 9.2 s of a configs[3] run, cuFFT 10.6 s)
     for (int d = 0; d < 3; d++)
-        if (!is_pow2(g.N[d]) || g.N[d] < 16 || g.N[d] > (force ? 1024 : 512)) return false;
+        if (!is_pow2(g.N[d]) || g.N[d] < 16 || g.N[d] > 1024) return false;
     return true;
 }
 

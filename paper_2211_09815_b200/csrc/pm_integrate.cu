@@ -230,4 +230,58 @@ int fill_zero(pm_ctx *c, void *ptr, size_t bytes)
     return PM_OK;
 }
 
+// ---- reductions and updates of the run with observations / the Omega_m gradient (eq. 49 last lines, eq. 51) ----------
+// sum_j a_j b_j in fp64, per-block partials then one fixed-order sum: acc[0] += coef * sum (bit-reproducible)
+__global__ void __launch_bounds__(256) dot_kernel(long long n, const float *__restrict__ a, const float *__restrict__ b,
+                                                  const long long *__restrict__ bfix, double bscale, double *__restrict__ partial)
+{
+    __shared__ double red[8];
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    double part = 0.0;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride)
+        part += (double)a[i] * (bfix ? (double)bfix[i] * bscale : (double)b[i]);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = part;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+        for (int k = 0; k < 8; k++) t += red[k];
+        partial[blockIdx.x] = t;
+    }
+}
+__global__ void dot_final_kernel(int nblocks, const double *__restrict__ partial, double coef, double *__restrict__ acc)
+{
+    if (threadIdx.x == 0 && blockIdx.x == 0) {
+        double t = 0.0;
+        for (int k = 0; k < nblocks; k++) t += partial[k];
+        acc[0] += coef * t;
+    }
+}
+__global__ void __launch_bounds__(256) axpy_kernel(long long n, float w, const float *__restrict__ src, float *__restrict__ dst)
+{
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) dst[i] = fmaf(w, src[i], dst[i]);
+}
+
+// acc[0] += coef * sum_j a_j b_j over the 3 N_p components; b is a float array, or (bfix) the fixed-point momenta
+int dot_accumulate(pm_ctx *c, const float *a, const float *b, const long long *bfix, double coef, double *acc)
+{
+    const long long n3 = 3 * c->g.np;
+    const int nb = ew_blocks(n3);
+    dot_kernel<<<nb, 256, 0, c->stream>>>(n3, a, b, bfix, ldexp(1.0, -PBITS), c->scal + 1);
+    dot_final_kernel<<<1, 32, 0, c->stream>>>(nb, c->scal + 1, coef, acc);
+    c->n_own += 2;
+    PM_LAUNCH_CHECK(c, "dot_kernel");
+    return PM_OK;
+}
+
+int axpy(pm_ctx *c, long long n, float w, const float *src, float *dst)
+{
+    axpy_kernel<<<ew_blocks(n), 256, 0, c->stream>>>(n, w, src, dst);
+    c->n_own++;
+    PM_LAUNCH_CHECK(c, "axpy_kernel");
+    return PM_OK;
+}
+
 }  // namespace pm

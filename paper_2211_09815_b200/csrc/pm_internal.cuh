@@ -264,5 +264,7 @@ int kick_drift_adj(pm_ctx *c, double K, double D);
 int objective_residual(pm_ctx *c, float *mesh, const float *target, double nbar);
 int combine_dJ_ds0(pm_ctx *c, float *out);
 int fill_zero(pm_ctx *c, void *ptr, size_t bytes);
+int dot_accumulate(pm_ctx *c, const float *a, const float *b, const long long *bfix, double coef, double *acc);
+int axpy(pm_ctx *c, long long n, float w, const float *src, float *dst);
 
 }  // namespace pm
