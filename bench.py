@@ -369,6 +369,17 @@ def run_ours(args):
     del s0, p0, target
 
     # ================= sub-records (N = 1 only; each guarded, a failure is recorded, not fatal) =================
+    if rank == 0 and world == 1 and not args.no_modes:
+        try:
+            line["modes"] = {"fp64_transforms": mode_fp64_transforms(args, torch, binding, p_over_s)}
+        except Exception as e:  # noqa: BLE001
+            line["modes"] = {"fp64_transforms": {"error": f"{type(e).__name__}: {e}"}}
+        torch.cuda.empty_cache()
+        try:
+            line["next_rows"] = next_rows_cfg1(torch, binding, p_over_s)
+        except Exception as e:  # noqa: BLE001
+            line["next_rows"] = {"error": f"{type(e).__name__}: {e}"}
+        torch.cuda.empty_cache()
     if rank == 0 and world == 1 and args.config == 2:
         if not args.no_scale_up:
             try:
@@ -386,6 +397,68 @@ def run_ours(args):
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
+
+
+def _events_ms(torch, fn, reps=1):
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(reps):
+        fn()
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) / reps
+
+
+def mode_fp64_transforms(args, torch, binding, p_over_s):
+    """The headline workload in the PM_FLAG_FP64_TRANSFORMS mode (transforms and k-space operators in fp64: the mode that
+    meets north_star's 1e-3 gradient bar at configs[1], tests/test_gpu_full_size.py): 1 warm-up + 2 timed runs."""
+    cfg, s0, p0, target = make_inputs(args.config, p_over_s)
+    npart = s0.shape[0]
+    pm = binding.PM(cfg["mesh"], cfg["lattice"], cfg["omega_m"], cfg["a"], flags=binding.PM_FLAG_FP64_TRANSFORMS)
+    dv = [torch.from_numpy(v).cuda() for v in (s0, p0, target)]
+    outs = {k: torch.empty((npart, 3), dtype=torch.float32, device="cuda") for k in ("s_n", "p_n", "xi0", "pi0", "dJ_ds0")}
+    J = [0.0]
+
+    def step():
+        J[0] = pm.run_fwd_adj(*dv, out=outs)["J"]
+
+    step()
+    ms = _events_ms(torch, step, 2)
+    rec = {"workload": cfg["name"], "value": npart * cfg["n_steps"] / (ms * 1e-3), "unit": UNIT, "ms_per_step": ms, "steps": 2,
+           "warmup": 1, "workspace_GB": pm.workspace_nbytes / 1e9, "objective_J": J[0],
+           "note": "transforms via cuFFT D2Z/Z2D + fp64 k-space kernels; all particle and mesh arrays fp32"}
+    pm.close()
+    return rec
+
+
+def next_rows_cfg1(torch, binding, p_over_s):
+    """SURVEY 8f rows at configs[1]'s sizes, milliseconds per call (CUDA events, 1 warm-up + 2 calls): the device IC
+    generator and its VJP (2LPT), the run with three observed snapshots and the Omega_m gradient, one Adam iteration."""
+    cfg, s0, p0, target = make_inputs(1, p_over_s)
+    npart = s0.shape[0]
+    pm = binding.PM(cfg["mesh"], cfg["lattice"], cfg["omega_m"], cfg["a"])
+    omega = torch.randn(cfg["lattice"], device="cuda", generator=torch.Generator(device="cuda").manual_seed(1))
+    xi, pi = torch.randn(npart, 3, device="cuda"), torch.randn(npart, 3, device="cuda")
+    amp = 0.05
+    rec = {"workload": cfg["name"]}
+    pm.ic_fwd(omega, amp)
+    rec["ic_fwd_2lpt_ms"] = _events_ms(torch, lambda: pm.ic_fwd(omega, amp), 2)
+    pm.ic_vjp(omega, amp, xi, pi)
+    rec["ic_vjp_2lpt_ms"] = _events_ms(torch, lambda: pm.ic_vjp(omega, amp, xi, pi), 2)
+    dv = [torch.from_numpy(v).cuda() for v in (s0, p0)]
+    n = cfg["n_steps"]
+    tg = torch.from_numpy(np.stack([target] * 3)).cuda()
+    steps, w = [n // 3, 2 * n // 3, n], [1.0, 1.0, 1.0]
+    pm.run_fwd_adj_obs(dv[0], dv[1], steps, w, tg)
+    rec["run_3_snapshots_ms"] = _events_ms(torch, lambda: pm.run_fwd_adj_obs(dv[0], dv[1], steps, w, tg), 2)
+    rec["run_3_snapshots_dJ_dOm_ms"] = _events_ms(torch, lambda: pm.run_fwd_adj_obs(dv[0], dv[1], steps, w, tg, want_dJ_dOm=True), 2)
+    pm.optimize_ic(omega, tg[0], amp, 1)
+    hist = []
+    rec["adam_iteration_ms"] = _events_ms(torch, lambda: hist.extend(pm.optimize_ic(omega, tg[0], amp, 2)), 1) / 2
+    rec["adam_J"] = hist
+    pm.close()
+    return rec
 
 
 def scale_up_cfg3(args, torch, binding, p_over_s, peak, peak_src, local):
@@ -537,6 +610,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-kernel-timing", action="store_true", help="no per-kernel CUDA events pass (debug)")
     ap.add_argument("--no-scale-up", action="store_true", help="skip the configs[3] sub-record")
+    ap.add_argument("--no-modes", action="store_true", help="skip the fp64-transform mode and the 8f-row timings")
     ap.add_argument("--no-sweep", action="store_true", help="skip the configs[4] sub-record")
     ap.add_argument("--sweep-lattice", type=int, default=512, help="particles per axis of the configs[4] kernel sweep (mesh = 2x)")
     args = ap.parse_args()

@@ -184,6 +184,20 @@ int pm_ic_vjp(pm_ctx *ctx, const float *dev_omega, double amp, double ns, double
 /* Host: out = {D1, D2, a^2 E D1', a^2 E D2'} at a0, the four time factors of eq. 2 (D2 by RK4 on eq. A1). */
 int pm_host_ic_factors(double omega_m, double a0, double out[4]);
 
+/* ---- optimisation of the initial conditions (the paper's second workload, Fig. 4) ----------------------
+ * One Adam update (Kingma & Ba 2015; the paper uses it with learning rate 0.1): t = 1, 2, ... is the iteration number,
+ * dev_m / dev_v the running first / second moments (zero before t = 1), all arrays [n] floats. */
+int pm_adam_step(pm_ctx *ctx, int64_t n, float *dev_w, const float *dev_g, float *dev_m, float *dev_v, int t, double lr,
+                 double beta1, double beta2, double eps);
+/* n_iter iterations of  omega -> pm_ic_fwd -> pm_run_fwd_adj (J, xi0, pi0) -> pm_ic_vjp (dJ/d omega) -> Adam(lr, 0.9,
+ * 0.999, 1e-8) on the white-noise field dev_omega[Lx][Ly][Lz] (updated in place), towards dev_delta_target (the mesh
+ * objective of pm_objective).  host_J_history[n_iter] (may be NULL) receives J BEFORE each update.  dev_scratch: at least
+ * pm_optimize_ic_scratch_bytes(ctx) bytes of device memory owned by the caller.  Synchronises once per iteration (J).
+ * No checkpoints are needed (L371, L381): the reverse pass retraces the forward one bit for bit. */
+size_t pm_optimize_ic_scratch_bytes(const pm_ctx *ctx);
+int pm_optimize_ic(pm_ctx *ctx, float *dev_omega, const float *dev_delta_target, double amp, double ns, double rc, int order,
+                   int n_iter, double lr, void *dev_scratch, size_t scratch_bytes, double *host_J_history);
+
 /* ---- instrumentation ---------------------------------------------------------------------------------
  * When enabled, every kernel launch / cuFFT call of the library is bracketed by CUDA events on the
  * ctx's stream.  pm_timing_read SYNCHRONISES, sums the elapsed time per kernel class since the last

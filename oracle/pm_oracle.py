@@ -333,3 +333,28 @@ def run_fwd_adj_obs(N, L, omega_m, a, s0, p0, obs_steps, obs_weights, targets, d
                                   _d(out["xi0"]), _d(out["pi0"]), _d(J_obs), _d(dth))
     out.update(J=J, J_obs=J_obs, dJ_dOm=float(dth[0]))
     return out
+
+
+# ---- Adam and the optimisation loop of the paper's Fig. 4 (L482-488), written out plainly (numpy, fp64) ----
+def adam_step(w, g, m, v, t, lr=0.1, beta1=0.9, beta2=0.999, eps=1e-8):
+    """Kingma & Ba (2015), Algorithm 1; returns the new (w, m, v).  t = 1, 2, ..."""
+    m = beta1 * m + (1.0 - beta1) * g
+    v = beta2 * v + (1.0 - beta2) * g * g
+    mhat = m / (1.0 - beta1 ** t)
+    vhat = v / (1.0 - beta2 ** t)
+    return w - lr * mhat / (np.sqrt(vhat) + eps), m, v
+
+
+def optimize_ic(N, L, omega_m, a, omega, target, amp, n_iter, lr=0.1, order=2, ns=-1.5, rc=2.0):
+    """omega -> ic -> run_fwd_adj -> ic_vjp -> Adam, n_iter times; returns (omega_final, J history before each update)."""
+    w = _f64(omega).reshape(-1).copy()
+    m = np.zeros_like(w)
+    v = np.zeros_like(w)
+    hist = []
+    for t in range(1, n_iter + 1):
+        s0, p0 = ic(N, L, omega_m, a[0], amp, w.reshape(L), order=order, ns=ns, rc=rc)
+        out = run_fwd_adj(N, L, omega_m, a, s0, p0, target)
+        g = ic_vjp(N, L, omega_m, a[0], amp, w.reshape(L), out["xi0"], out["pi0"], order=order, ns=ns, rc=rc)
+        hist.append(out["J"])
+        w, m, v = adam_step(w, g, m, v, t, lr)
+    return w.reshape(L), hist

@@ -57,6 +57,9 @@ _SIGS = {
     "pm_ic_vjp": (_int, [_vp, _vp, _dbl, _dbl, _dbl, _int, _vp, _vp, _vp]),
     "pm_run_fwd_adj_obs": (_int, [_vp, _vp, _vp, _int, C.POINTER(C.c_int32), C.POINTER(_dbl), _vp, _vp, _vp,
                                   C.POINTER(_dbl), C.POINTER(_dbl), _vp, _vp, _vp, C.POINTER(_dbl)]),
+    "pm_adam_step": (_int, [_vp, _i64, _vp, _vp, _vp, _vp, _int, _dbl, _dbl, _dbl, _dbl]),
+    "pm_optimize_ic_scratch_bytes": (C.c_size_t, [_vp]),
+    "pm_optimize_ic": (_int, [_vp, _vp, _vp, _dbl, _dbl, _dbl, _int, _int, _dbl, _vp, C.c_size_t, C.POINTER(_dbl)]),
     "pm_scatter": (_int, [_vp, _i64, _vp, _vp, _int, _vp]),
     "pm_gather": (_int, [_vp, _i64, _vp, _vp, _int, _vp]),
     "pm_gather_grad": (_int, [_vp, _i64, _vp, _vp, _int, _vp, _vp]),
@@ -266,6 +269,20 @@ class PM:
                                             C.byref(dth) if want_dJ_dOm else None), "pm_run_fwd_adj_obs")
         out.update(J=J.value, J_obs=list(Jk), dJ_dOm=dth.value if want_dJ_dOm else None)
         return out
+
+    # ---- optimisation of the initial conditions (Fig. 4) ----
+    def adam_step(self, w, g, m, v, t, lr=0.1, beta1=0.9, beta2=0.999, eps=1e-8):
+        self._check(_lib.pm_adam_step(self._h, w.numel(), _ptr(w, "w"), _ptr(g, "g"), _ptr(m, "m"), _ptr(v, "v"), int(t),
+                                      float(lr), float(beta1), float(beta2), float(eps)), "pm_adam_step")
+
+    def optimize_ic(self, omega, target, amp, n_iter, lr=0.1, order=2, ns=-1.5, rc=2.0):
+        """n_iter Adam iterations on the white noise omega (updated in place); returns the J history"""
+        nb = _lib.pm_optimize_ic_scratch_bytes(self._h)
+        scratch = torch.empty(nb, dtype=torch.uint8, device=self.device)
+        hist = (_dbl * max(int(n_iter), 1))()
+        self._check(_lib.pm_optimize_ic(self._h, _ptr(omega, "omega"), _ptr(target, "target"), float(amp), float(ns), float(rc),
+                                        int(order), int(n_iter), float(lr), scratch.data_ptr(), nb, hist), "pm_optimize_ic")
+        return list(hist)[: int(n_iter)]
 
     # ---- initial conditions (eq. 2-6) and dJ/d(omega) (eq. 51) ----
     def ic_fwd(self, omega, amp, order=2, ns=-1.5, rc=2.0):

@@ -266,5 +266,6 @@ int combine_dJ_ds0(pm_ctx *c, float *out);
 int fill_zero(pm_ctx *c, void *ptr, size_t bytes);
 int dot_accumulate(pm_ctx *c, const float *a, const float *b, const long long *bfix, double coef, double *acc);
 int axpy(pm_ctx *c, long long n, float w, const float *src, float *dst);
+int adam_step(pm_ctx *c, long long n, float *w, const float *g, float *m, float *v, int t, double lr, double b1, double b2, double eps);
 
 }  // namespace pm
