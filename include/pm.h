@@ -2,7 +2,7 @@
  * pm.h -- C ABI of libpm: the data-parallel hot path of the adjoint particle-mesh method of
  * "Differentiable Cosmological Simulation with the Adjoint Method" (arxiv 2211.09815),
  * hand-written CUDA for sm_100a (B200).  The 3-D transforms are the library's own passes on power-of-two
- * meshes up to 512 per axis (k-space operators fused in) and cuFFT's on every other mesh.
+ * meshes from 16 to 1024 per axis (k-space operators fused in) and cuFFT's on every other mesh.
  *
  * Citations are /root/reference/PAPER.md line numbers (L..) with the equation they fall in.
  *
