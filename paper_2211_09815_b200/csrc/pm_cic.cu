@@ -464,9 +464,10 @@ struct ScatterSlot {
     int pool;                   // heavy tile: slot of the global integer accumulator the chunks are combined in; else -1
 };
 
-// record stages: 4 for the scalar scatter (48 KB per CTA), 2 for three components (64 KB: three CTAs per SM)
+// record stages: 3 for the scalar scatter (40 KB per CTA: five CTAs per SM at 40 registers), 2 for three components
+// (64 KB: three CTAs per SM)
 template <int C>
-constexpr int scatter_stages() { return C == 1 ? 4 : 2; }
+constexpr int scatter_stages() { return C == 1 ? 3 : 2; }
 template <int C>
 constexpr size_t scatter_smem_bytes() { return (size_t)2 * C * TILE_PTS * sizeof(int) + (size_t)scatter_stages<C>() * RCAP * sizeof(uint4); }
 
@@ -475,7 +476,7 @@ __global__ void __launch_bounds__(NTHREADS) scatter_kernel(const __grid_constant
                                                            const uint4 *__restrict__ rec, const int *__restrict__ offsets,
                                                            const float *__restrict__ val, float *__restrict__ mesh)
 {
-    constexpr int NST = C == 1 ? 4 : 2;  // = scatter_stages<C>()
+    constexpr int NST = C == 1 ? 3 : 2;  // = scatter_stages<C>()
     extern __shared__ __align__(128) unsigned char dsm[];
     typedef int AccBuf[C][TILE_PTS];
     AccBuf *acc = reinterpret_cast<AccBuf *>(dsm);                                        // [2]
@@ -870,6 +871,11 @@ __global__ void __launch_bounds__(NTHREADS) scatter_kernel(const __grid_constant
                 } else if (mq == 0) {
                     f = make_float4((float)(unsigned)a.x * inv_scale, (float)(unsigned)a.y * inv_scale,
                                     (float)(unsigned)a.z * inv_scale, (float)(unsigned)a.w * inv_scale);
+                } else if ((a.x | a.y | a.z | a.w) >= 0 && mq < (1ll << 30)) {
+                    // all four below 2^31 (every point but the densest): the exact difference fits in 32 bits
+                    const int m32 = (int)mq;
+                    f = make_float4((float)(a.x - m32) * inv_scale - mrest, (float)(a.y - m32) * inv_scale - mrest,
+                                    (float)(a.z - m32) * inv_scale - mrest, (float)(a.w - m32) * inv_scale - mrest);
                 } else {
                     f = make_float4((float)((long long)(unsigned)a.x - mq) * inv_scale - mrest, (float)((long long)(unsigned)a.y - mq) * inv_scale - mrest,
                                     (float)((long long)(unsigned)a.z - mq) * inv_scale - mrest, (float)((long long)(unsigned)a.w - mq) * inv_scale - mrest);

@@ -287,13 +287,13 @@ int axpy(pm_ctx *c, long long n, float w, const float *src, float *dst)
 // Adam (the optimiser of the paper's Fig. 4 experiment, L482-488): m <- b1 m + (1 - b1) g, v <- b2 v + (1 - b2) g^2,
 // w <- w - lr (m / (1 - b1^t)) / (sqrt(v / (1 - b2^t)) + eps); c1 = 1 / (1 - b1^t), c2 = 1 / (1 - b2^t) from the host
 __global__ void __launch_bounds__(256) adam_kernel(long long n, float *__restrict__ w, const float *__restrict__ g, float *__restrict__ m,
-                                                   float *__restrict__ v, float lr, float b1, float b2, float eps, float c1, float c2)
+                                                   float *__restrict__ v, float lr, float b1, float b2, float omb1, float omb2, float eps, float c1, float c2)
 {
     const long long stride = (long long)gridDim.x * blockDim.x;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
         const float gi = g[i];
-        const float mi = b1 * m[i] + (1.f - b1) * gi;
-        const float vi = b2 * v[i] + (1.f - b2) * gi * gi;
+        const float mi = b1 * m[i] + omb1 * gi;          // omb = 1 - beta, formed in fp64 on the host (1 - 0.999f is off by 5e-5)
+        const float vi = b2 * v[i] + omb2 * gi * gi;
         m[i] = mi;
         v[i] = vi;
         w[i] -= lr * (mi * c1) / (sqrtf(vi * c2) + eps);
@@ -303,7 +303,7 @@ __global__ void __launch_bounds__(256) adam_kernel(long long n, float *__restric
 int adam_step(pm_ctx *c, long long n, float *w, const float *g, float *m, float *v, int t, double lr, double b1, double b2, double eps)
 {
     const double c1 = 1.0 / (1.0 - pow(b1, (double)t)), c2 = 1.0 / (1.0 - pow(b2, (double)t));
-    adam_kernel<<<ew_blocks(n), 256, 0, c->stream>>>(n, w, g, m, v, (float)lr, (float)b1, (float)b2, (float)eps, (float)c1, (float)c2);
+    adam_kernel<<<ew_blocks(n), 256, 0, c->stream>>>(n, w, g, m, v, (float)lr, (float)b1, (float)b2, (float)(1.0 - b1), (float)(1.0 - b2), (float)eps, (float)c1, (float)c2);
     c->n_own++;
     PM_LAUNCH_CHECK(c, "adam_kernel");
     return PM_OK;

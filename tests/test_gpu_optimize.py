@@ -32,8 +32,8 @@ def test_adam_step_parity(pmlib, orc):
     wo, mo, vo = orc.adam_step(w.astype(np.float64), g.astype(np.float64), m.astype(np.float64), v.astype(np.float64), 5, lr=0.1)
     # the update is lr * m_hat / (sqrt(v_hat) + eps), up to 30 here where v is tiny: compare the STEP, fp32 against fp64
     np.testing.assert_allclose(wd.cpu().numpy().astype(np.float64) - w, wo - w, rtol=2e-5, atol=2e-6)
-    np.testing.assert_allclose(md.cpu().numpy(), mo, rtol=1e-6, atol=1e-7)
-    np.testing.assert_allclose(vd.cpu().numpy(), vo, rtol=1e-6, atol=1e-9)
+    np.testing.assert_allclose(md.cpu().numpy(), mo, rtol=2e-6, atol=1e-7)
+    np.testing.assert_allclose(vd.cpu().numpy(), vo, rtol=2e-6, atol=1e-9)
     pm.close()
 
 
