@@ -44,13 +44,14 @@ PLAN_MESHES = [
 ]
 
 
-@pytest.mark.parametrize("mesh", PLAN_MESHES)
-@pytest.mark.parametrize("deconv", [0, 1])
+# deconvolution is covered on three of the plans (a 512, a 1024 x axis and a 1024 z axis)
+PLAN_CASES = [(m, 0) for m in PLAN_MESHES] + [((512, 16, 32), 1), ((16, 32, 1024), 1), ((1024, 16, 16), 1)]
+
+
+@pytest.mark.parametrize("mesh,deconv", PLAN_CASES)
 def test_own_fft_plans_against_oracle(pmlib, orc, mesh, deconv, monkeypatch):
     """pm_force / pm_force_vjp through the own z, y and fused x passes against the oracle (eq. 11 L127-131 and its
     transpose), rel L2 <= 1e-5, on a mesh with one long axis per radix plan."""
-    if deconv and mesh not in ((512, 16, 32), (16, 32, 1024), (1024, 16, 16)):
-        pytest.skip("deconvolution is covered on three of the plans")
     monkeypatch.setenv("PM_FFT", "own")   # also above the default own-FFT size limit, if any
     lattice = tuple(n // 2 for n in mesh)
     rng = np.random.default_rng(41)
