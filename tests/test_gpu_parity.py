@@ -50,6 +50,13 @@ MESHES = [
 ]
 
 
+def max_err(a, b):
+    """largest element-wise error relative to the largest reference element (a single wrong element shows as O(1))"""
+    a = np.asarray(a, dtype=np.float64)
+    b = np.asarray(b, dtype=np.float64)
+    return float(np.max(np.abs(a - b)) / max(np.max(np.abs(b)), 1e-300))
+
+
 @pytest.mark.parametrize("mesh,lattice", MESHES)
 def test_scatter_gather_parity(pmlib, orc, mesh, lattice):
     rng = np.random.default_rng(11)
@@ -63,12 +70,14 @@ def test_scatter_gather_parity(pmlib, orc, mesh, lattice):
     rho = pm.scatter(xd).cpu().numpy()
     rho_o = orc.scatter(mesh, x)
     assert rel_l2(rho, rho_o) <= 1e-5
+    assert max_err(rho, rho_o) <= 1e-5                                 # element by element, not only in the norm
     assert abs(rho.astype(np.float64).sum() - n) <= 1e-5 * n          # P1 mass conservation
     # --- scatter with values, C = 3 and C = 1
     val = rng.standard_normal((n, 3)).astype(np.float32) * np.exp(rng.normal(0, 2, (n, 1))).astype(np.float32)
     m3 = pm.scatter(xd, dev(val)).cpu().numpy()
     m3_o = orc.scatter(mesh, x, val)
     assert rel_l2(m3, m3_o) <= 1e-5
+    assert max_err(m3, m3_o) <= 1e-5
     m1 = pm.scatter(xd, dev(val[:, :1].copy())).cpu().numpy()
     assert rel_l2(m1[0], m3_o[0]) <= 1e-5
     # --- gather C = 3, C = 1
@@ -77,6 +86,7 @@ def test_scatter_gather_parity(pmlib, orc, mesh, lattice):
     g3 = pm.gather(xd, fd).cpu().numpy()
     g3_o = orc.gather(mesh, x, f)
     assert rel_l2(g3, g3_o) <= 1e-5
+    assert max_err(g3, g3_o) <= 1e-5
     g1 = pm.gather(xd, fd[0].contiguous()).cpu().numpy()
     assert rel_l2(g1[:, 0], g3_o[:, 0]) <= 1e-5
     # --- weight-gradient gather: scalar mesh without cotangent, 3 meshes with cotangents
@@ -87,6 +97,7 @@ def test_scatter_gather_parity(pmlib, orc, mesh, lattice):
     gg3 = pm.gather_grad(xd, fd, dev(cot)).cpu().numpy()
     gg3_o = orc.gather_grad(mesh, x, f, cot)
     assert rel_l2(gg3, gg3_o) <= 1e-5
+    assert max_err(gg, gg_o) <= 1e-5 and max_err(gg3, gg3_o) <= 1e-5
     # --- transpose identity <S(x, v), f> = <v, G(x, f)> on the GPU results (P2)
     lhs = float(np.sum(m3.astype(np.float64) * f))
     rhs = float(np.sum(val.astype(np.float64) * g3))
