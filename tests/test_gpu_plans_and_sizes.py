@@ -200,6 +200,48 @@ def test_config3_force_vjp_own_fft_vs_cufft(pmlib, monkeypatch):
     assert np.all(tot <= 1e-5 * np.abs(res["own"][0]).sum(axis=0))      # P3 momentum conservation at full size
 
 
+def test_config3_whole_run_exact_reversal_and_fp64_transform_cross_check(pmlib):
+    """configs[3] (512^3 particles, 1024^3 mesh, 100 KDK steps) end to end.  The oracle cannot run this size on the box
+    (hours, ~70 GB per force), so what is checked is what holds at any size: (1) the reverse pass returns the quantised
+    initial state BIT FOR BIT at full size (134 M particles, 100 steps forward and back, own 1024-point transform passes);
+    (2) the fp32 path against the fp64-transform mode of the same library (the mode that sits within 1.7e-6 cell and 1.5e-4
+    of the oracle at configs[1]): final positions within north_star's 1e-4 cell rms, objective 1e-4,
+    median per-particle gradient difference 1e-3 on 65536 sampled particles.  A stand-in for the oracle, stated as such."""
+    free, _ = torch.cuda.mem_get_info()
+    cfg = inputs.config(3)
+    need = pmlib.workspace_bytes(cfg["mesh"], cfg["lattice"], cfg["omega_m"], cfg["a"], flags=pmlib.PM_FLAG_FP64_TRANSFORMS)
+    if free < need + (24 << 30):
+        pytest.fail(f"configs[3] in the fp64-transform mode needs {need / 2**30:.0f} GiB of workspace; {free / 2**30:.0f} GiB free")
+    s0 = inputs.zeldovich_displacement(cfg["lattice"], cfg["mesh"], seed=1, rms=0.3)
+    g = pmlib.host_growth(cfg["omega_m"], cfg["a"][0])
+    p0 = (s0.astype(np.float64) * (g[2] / g[0])).astype(np.float32)
+    target = inputs.lognormal_target(cfg["mesh"], seed=2, sigma=1.0)
+    dv = [torch.from_numpy(v).cuda() for v in (s0, p0, target)]
+    del target
+    idx = np.sort(np.random.default_rng(7).choice(s0.shape[0], size=65536, replace=False))
+    res = {}
+    for mode, flags in (("fp32", 0), ("fp64t", pmlib.PM_FLAG_FP64_TRANSFORMS)):
+        pm = pmlib.PM(cfg["mesh"], cfg["lattice"], cfg["omega_m"], cfg["a"], flags=flags)
+        out = pm.run_fwd_adj(*dv)
+        own, fft = pm.launch_count()
+        assert (fft == 0) == (mode == "fp32")             # the fp32 path runs its own transform passes at 1024^3
+        s_q = np.rint(s0.astype(np.float64) * 2.0 ** 32) / 2.0 ** 32
+        assert np.array_equal(out["s_rec"].cpu().numpy(), s_q.astype(np.float32)), f"{mode}: reverse integration is not exact"
+        res[mode] = {k: out[k].cpu().numpy()[idx].astype(np.float64) for k in ("s_n", "dJ_ds0")}
+        res[mode]["J"] = out["J"]
+        pm.close()
+        del out, pm
+        torch.cuda.empty_cache()
+    rms = float(np.sqrt(np.mean(np.sum((res["fp32"]["s_n"] - res["fp64t"]["s_n"]) ** 2, axis=1))))
+    a, b = res["fp32"]["dJ_ds0"], res["fp64t"]["dJ_ds0"]
+    e2, n2 = np.sum((a - b) ** 2, axis=1), np.sum(b ** 2, axis=1)
+    print(f"configs[3] fp32 vs fp64-transform mode: positions rms {rms:.3e} cell, J rel {abs(res['fp32']['J'] / res['fp64t']['J'] - 1):.2e}, "
+          f"dJ/ds0 rel L2 {np.sqrt(e2.sum() / n2.sum()):.3e}, median {np.median(np.sqrt(e2 / n2)):.3e}")
+    assert rms <= 1e-4
+    assert abs(res["fp32"]["J"] / res["fp64t"]["J"] - 1) <= 1e-4
+    assert np.median(np.sqrt(e2 / n2)) <= 1e-3
+
+
 @pytest.fixture(scope="module")
 def big(pmlib):
     """One ctx of the configs[3] geometry (69.5 GB workspace) shared by the full-size kernel tests."""
