@@ -268,20 +268,23 @@ def _subbox_scatter(orc, x, val, lo, size):
     return out[..., h:h + size, h:h + size, h:h + size], int(sel.sum())
 
 
-@pytest.mark.parametrize("order", ["generation", "random"])
-def test_config4_inputs_full_size_kernel_parity(pmlib, orc, big, order):
-    """The real configs[4] inputs (512^3 particles, 20000 blobs, 1024^3 mesh) in both memory orders: pm_scatter (unit mass)
+def test_config4_inputs_full_size_kernel_parity(pmlib, orc, big):
+    """The real configs[4] inputs (512^3 particles, 20000 blobs, 1024^3 mesh).  Generation order: pm_scatter (unit mass)
     against the oracle's serial scatter on the WHOLE mesh; the 3-component scatter on sub-boxes around the densest
-    cells and at the periodic corner; gathers and weight-gradient gathers on 20000 sampled particles.  This exercises
+    cells and at the periodic corner; gathers and weight-gradient gathers on 20000 sampled particles.  Random memory
+    order (the same particles permuted): every result must equal the generation-order one BIT FOR BIT -- the meshes
+    because the scatters accumulate in integers, the per-particle outputs because they depend on the particle alone --
+    which carries the oracle comparison over without a second 134 M-particle serial scatter on the host.  This exercises
     the 64-bit index paths, the 1024-axis tile counts and the work queues / accumulator pool at their real load."""
     pm = big
     mesh = (BIG_N,) * 3
     npart = BIG_L ** 3
-    x = inputs.blob_positions(npart, mesh, seed=3, n_blobs=20000, order=order)
+    x = inputs.blob_positions(npart, mesh, seed=3, n_blobs=20000, order="generation")
     xd = torch.from_numpy(x).cuda()
     rng = np.random.default_rng(23)
     # --- unit-mass scatter, whole mesh, compared slab by slab (the fp64 mesh of the oracle is 8.6 GB)
-    rho = pm.scatter(xd).cpu().numpy()
+    rho_d = pm.scatter(xd)
+    rho = rho_d.cpu().numpy()
     rho_o = orc.scatter(mesh, x)
     assert rho_o.max() > 100.0
     num = den = tot = 0.0
@@ -308,18 +311,35 @@ def test_config4_inputs_full_size_kernel_parity(pmlib, orc, big, order):
         ix = [torch.from_numpy((np.arange(32) + lo[d]) % BIG_N).cuda() for d in range(3)]
         got = m3[:, ix[0]][:, :, ix[1]][:, :, :, ix[2]].cpu().numpy()
         assert nsel > 0 and rel_l2(got, ref) <= 1e-5, f"box {lo}"
-    del m3, vd
+    del val
+    # --- the same particles in random memory order: bit-identical meshes
+    perm = torch.from_numpy(np.random.default_rng(29).permutation(npart)).cuda()
+    xr = xd[perm].contiguous()
+    assert torch.equal(pm.scatter(xr), rho_d), "unit-mass scatter depends on the memory order"
+    del rho_d
+    vr = vd[perm].contiguous()
+    del vd
+    m3r = pm.scatter(xr, vr)
+    assert torch.equal(m3r, m3), "valued scatter depends on the memory order"
+    del m3, m3r, vr
     torch.cuda.empty_cache()
-    # --- gathers on sampled particles
+    # --- gathers on sampled particles (generation order against the oracle, random order against generation order)
     gen = torch.Generator(device="cuda").manual_seed(5)
     fd = torch.randn((3,) + mesh, device="cuda", generator=gen)
     idx = np.sort(rng.choice(npart, 20000, replace=False))
-    g3 = pm.gather(xd, fd)[torch.from_numpy(idx).cuda()].cpu().numpy()
+    g3d = pm.gather(xd, fd)
+    g3 = g3d[torch.from_numpy(idx).cuda()].cpu().numpy()
     f = fd.cpu().numpy()
     assert rel_l2(g3, orc.gather(mesh, x[idx], f)) <= 1e-5
+    assert torch.equal(pm.gather(xr, fd), g3d[perm]), "gather depends on the memory order"
+    del g3d
     cot = rng.standard_normal((npart, 3)).astype(np.float32)
-    gg = pm.gather_grad(xd, fd, torch.from_numpy(cot).cuda())[torch.from_numpy(idx).cuda()].cpu().numpy()
+    cd = torch.from_numpy(cot).cuda()
+    ggd = pm.gather_grad(xd, fd, cd)
+    gg = ggd[torch.from_numpy(idx).cuda()].cpu().numpy()
     assert rel_l2(gg, orc.gather_grad(mesh, x[idx], f, cot[idx])) <= 1e-5
+    assert torch.equal(pm.gather_grad(xr, fd, cd[perm].contiguous()), ggd[perm]), "weight-gradient gather depends on the memory order"
+    del ggd, cd
     gs = pm.gather_grad(xd, fd[0].contiguous())[torch.from_numpy(idx).cuda()].cpu().numpy()
     assert rel_l2(gs, orc.gather_grad(mesh, x[idx], f[0])) <= 1e-5
     pm.get_objective()   # synchronises and checks the work-queue watchdog
