@@ -381,7 +381,7 @@ struct XPlan {
     }
 };
 
-#define PM_X_MINBLOCKS(NX) ((NX) >= 1024 ? 2 : ((NX) >= 512 ? 3 : 2))
+#define PM_X_MINBLOCKS(NX, CS) ((NX) >= 1024 ? 2 : ((NX) >= 512 ? ((CS) == 4 ? 2 : 3) : 2))
 
 // T(position, column) -> f_y = i kt_y T and f_z = i kt_z T (kt_z of the thread's own column: a thread only ever sees one)
 struct StoreYZ {
@@ -399,7 +399,7 @@ struct StoreYZ {
 // ---- x pass fused with the force operator: rho(k) -> f_d(k) = i kt_d G rho(k), d = 1..3, back-transformed along x ----
 // grid = (column tiles along z, Ny); shared: one tile + Nx twiddles + the x-dependent k tables
 template <int NX, int CS>
-__global__ void __launch_bounds__(FFT_T, PM_X_MINBLOCKS(NX)) fft_x_force_kernel(FftGeom g, const float2 *rho, float2 *f)
+__global__ void __launch_bounds__(FFT_T, PM_X_MINBLOCKS(NX, CS)) fft_x_force_kernel(FftGeom g, const float2 *rho, float2 *f)
 {
     typedef XPlan<NX, CS> P;
     constexpr int B = P::B, RL = P::RL, IT = P::IT;
@@ -471,7 +471,7 @@ __global__ void __launch_bounds__(FFT_T, PM_X_MINBLOCKS(NX)) fft_x_force_kernel(
 
 // ---- x pass fused with the adjoint operator: psi(k) = -i G sum_d kt_d Pi_d(k), back-transformed along x ----------
 template <int NX, int CS>
-__global__ void __launch_bounds__(FFT_T, PM_X_MINBLOCKS(NX)) fft_x_adjoint_kernel(FftGeom g, const float2 *Pi, float2 *psi)
+__global__ void __launch_bounds__(FFT_T, PM_X_MINBLOCKS(NX, CS)) fft_x_adjoint_kernel(FftGeom g, const float2 *Pi, float2 *psi)
 {
     typedef XPlan<NX, CS> P;
     constexpr int B = P::B, RL = P::RL, IT = P::IT;
@@ -802,7 +802,7 @@ int fft_own_init(pm_ctx *c)
         case 64: CASE(64, 4); break;    \
         case 128: CASE(128, 4); break;  \
         case 256: CASE(256, 4); break;  \
-        case 512: CASE(512, 3); break;  \
+        case 512: CASE(512, 4); break;  \
         case 1024: CASE(1024, 3); break; \
         default: return fail(c, PM_EINVAL, "own FFT", "unsupported axis length"); \
     }
@@ -814,7 +814,7 @@ int fft_own_init(pm_ctx *c)
         case 64: CASE(64, 4); break;    \
         case 128: CASE(128, 4); break;  \
         case 256: CASE(256, 4); break;  \
-        case 512: CASE(512, 3); break;  \
+        case 512: CASE(512, 4); break;  \
         case 1024: CASE(1024, 3); break; \
         default: return fail(c, PM_EINVAL, "own FFT", "unsupported axis length"); \
     }
@@ -825,7 +825,8 @@ static int fft_z(pm_ctx *c, float *mesh, int nb, bool inverse)
     FftGeom fg = *geom_of(c);
     const int M = g.N[2] / 2;
     long long nrows = (long long)nb * g.N[0] * g.N[1];
-    const int ZRS = M >= 512 ? 3 : 4, ZROWS = 1 << ZRS, ZP = ZROWS + 1;  // fewer rows per CTA for long rows: 3 CTAs per SM
+    // 16 rows per CTA, 8 for the longest rows (2 CTAs per SM at Nz = 1024); 8 rows at Nz = 512 were measured slower (0.48 -> 0.53 ms)
+    const int ZRS = M >= 512 ? 3 : 4, ZROWS = 1 << ZRS, ZP = ZROWS + 1;
     unsigned grid = (unsigned)((nrows + ZROWS - 1) / ZROWS);
     size_t second = (size_t)(M + 1) * ZP;                       // outb / inb: transposed [M + 1][ZP] or row-major staging
     if (second < (size_t)ZROWS * (g.zs / 2)) second = (size_t)ZROWS * (g.zs / 2);
@@ -854,7 +855,9 @@ static int fft_y(pm_ctx *c, float *mesh, int nb, bool inverse)
 {
     const Geometry &g = c->g;
     FftGeom fg = *geom_of(c);
-    const int cs = g.N[1] <= 256 ? 4 : 3, B = 1 << cs;
+    // 16 columns (128-byte pieces) up to 512 points: 0.445 -> 0.394 ms per launch at 512^3 against 8 columns; at 1024 a
+    // 16-column tile is 128 KB (one CTA per SM) and loses (3.9 -> 5.1 ms): 8 columns there
+    const int cs = g.N[1] <= 512 ? 4 : 3, B = 1 << cs;
     dim3 grid((unsigned)((fg.zsc + B - 1) / B), (unsigned)g.N[0], (unsigned)nb);
     size_t smem = sizeof(float2) * ((size_t)g.N[1] + (size_t)g.N[1] * B);
     Timer t(c, TC_FFT_Y, 16.0 * (double)g.nk * nb);
@@ -872,7 +875,9 @@ static int fft_x_fused(pm_ctx *c, const float *in, float *out, double nbar, bool
     const Geometry &g = c->g;
     FftGeom fg = *geom_of(c);
     fg.c0 = 1.5 * c->prm.omega_m / (nbar * (double)g.ng);
-    const int cs = g.N[0] <= 256 ? 4 : 3, B = 1 << cs;  // one tile of Nx x B: 64-byte pieces at 512 and 1024
+    // one tile of Nx x B: 16 columns (128-byte pieces) up to 512 points (0.76 -> 0.71 ms at 512^3 against 8 columns, two CTAs
+    // per SM at 128 registers), 8 columns at 1024
+    const int cs = g.N[0] <= 512 ? 4 : 3, B = 1 << cs;
     dim3 grid((unsigned)((fg.zsc + B - 1) / B), (unsigned)g.N[1]);
     size_t smem = sizeof(float2) * ((size_t)g.N[0] + (size_t)g.N[0] * B) + (2 * sizeof(double) + sizeof(float)) * (size_t)g.N[0];
     Timer t(c, adjoint ? TC_KSPACE_ADJ : TC_KSPACE_FORCE, 32.0 * (double)g.nk);

@@ -9,6 +9,8 @@
     mesh (unit mass) and on sub-boxes (3 components), gathers on sampled particles, for the real configs[4] inputs;
     own-FFT path against the cuFFT path for pm_force / pm_force_vjp at 1024^3.
 """
+import gc
+
 import numpy as np
 import pytest
 
@@ -207,6 +209,8 @@ def test_config3_whole_run_exact_reversal_and_fp64_transform_cross_check(pmlib):
     (2) the fp32 path against the fp64-transform mode of the same library (the mode that sits within 1.7e-6 cell and 1.5e-4
     of the oracle at configs[1]): final positions within north_star's 1e-4 cell rms, objective 1e-4,
     median per-particle gradient difference 1e-3 on 65536 sampled particles.  A stand-in for the oracle, stated as such."""
+    gc.collect()
+    torch.cuda.empty_cache()            # blocks cached by the earlier tests of this process count as used otherwise
     free, _ = torch.cuda.mem_get_info()
     cfg = inputs.config(3)
     need = pmlib.workspace_bytes(cfg["mesh"], cfg["lattice"], cfg["omega_m"], cfg["a"], flags=pmlib.PM_FLAG_FP64_TRANSFORMS)
@@ -245,6 +249,8 @@ def test_config3_whole_run_exact_reversal_and_fp64_transform_cross_check(pmlib):
 @pytest.fixture(scope="module")
 def big(pmlib):
     """One ctx of the configs[3] geometry (69.5 GB workspace) shared by the full-size kernel tests."""
+    gc.collect()
+    torch.cuda.empty_cache()
     free, _ = torch.cuda.mem_get_info()
     need = pmlib.workspace_bytes((BIG_N,) * 3, (BIG_L,) * 3, 0.3, [1.0])
     if free < need + (24 << 30):
