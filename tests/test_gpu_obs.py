@@ -65,3 +65,19 @@ def test_single_final_observation_equals_the_plain_run(pmlib, orc):
     for k in ("s_n", "p_n", "xi0", "pi0", "dJ_ds0"):
         assert torch.equal(obs[k], plain[k]), k
     pm.close()
+
+
+def test_observation_of_the_initial_snapshot(pmlib, orc):
+    """an observation at t_0 is added after the last adjoint step (O_0): xi_0 then contains dJ_0/dx_0 directly"""
+    mesh, lattice, omm = (32, 32, 32), (16, 16, 16), 0.3
+    a = inputs.a_schedule(1.0 / 8, 4)
+    steps, w = [0, 4], [1.5, 1.0]
+    s0, p0, targets = _inputs(orc, mesh, lattice, omm, a, 2)
+    ref = orc.run_fwd_adj_obs(mesh, lattice, omm, a, s0, p0, steps, w, targets)
+    pm = pmlib.PM(mesh, lattice, omm, a)
+    out = pm.run_fwd_adj_obs(dev(s0), dev(p0), steps, w, dev(targets), want_dJ_dOm=True)
+    np.testing.assert_allclose(out["J_obs"], ref["J_obs"], rtol=1e-4)
+    assert rel_l2(out["xi0"].cpu().numpy(), ref["xi0"]) <= 1e-3
+    assert rel_l2(out["pi0"].cpu().numpy(), ref["pi0"]) <= 1e-3
+    assert abs(out["dJ_dOm"] - ref["dJ_dOm"]) <= 1e-3 * abs(ref["dJ_dOm"])
+    pm.close()
