@@ -105,7 +105,7 @@ def test_config1_full_run_fp64_transforms_meets_every_bar(pmlib):
 def _run_against_golden(pmlib, k, flags):
     path = os.path.join(GOLDEN, f"run_cfg{k}.npz")
     if not os.path.exists(path):
-        pytest.skip(f"{path} is missing: write it with `python tests/golden/make_golden_run.py {k}` (oracle only, hours)")
+        pytest.fail(f"{path} is missing: write it with `python tests/golden/make_golden_run.py {k}` (oracle only, hours)")
     gold = np.load(path)
     cfg = inputs.config(k)
     s0 = inputs.zeldovich_displacement(cfg["lattice"], cfg["mesh"], seed=1, rms=0.3)
