@@ -123,16 +123,21 @@ def test_config2_full_run_against_stored_oracle(pmlib):
     objective and exact reversal at north_star's numbers; the fp32 path's gradient is reported against the bar it is
     held to at configs[1] (reading R27) and the fp64-transform mode must meet 1e-3 untrimmed."""
     gold, s0, out = _run_against_golden(pmlib, 2, 0)
-    _check_forward_and_reversal(gold, s0, out)
+    rms = _check_forward_and_reversal(gold, s0, out)
+    print(f"configs[2] fp32 path: final positions rms {rms:.3e} cell")
     for k in ("xi0", "pi0", "dJ_ds0"):
         e, e_trim, e_med = _gradient_errors(gold, out, k)
         print(f"configs[2] fp32 path {k}: rel L2 {e:.3e}, without the worst 1 % {e_trim:.3e}, median {e_med:.3e}")
+        # measured 2.1-2.6e-3 / 1.5e-4 / 2.0e-4 (reading R27: the fp32 transforms; a handful of particles in collapsed
+        # clumps carry the squared error): held to the measured value x 1.5 and, without the worst 1 %, to north_star's 1e-3
+        assert e <= 3.9e-3, f"{k} rel L2 {e}"
+        assert e_trim <= 1e-3, f"{k} rel L2 without the worst 1% {e_trim}"
         assert e_med <= 1e-3, f"{k} median per-particle relative error {e_med}"
-        assert e_trim <= 2e-3, f"{k} rel L2 without the worst 1% {e_trim}"
     del out
     torch.cuda.empty_cache()
     gold, s0, out = _run_against_golden(pmlib, 2, pmlib.PM_FLAG_FP64_TRANSFORMS)
-    _check_forward_and_reversal(gold, s0, out)
+    rms = _check_forward_and_reversal(gold, s0, out)
+    print(f"configs[2] fp64 transforms: final positions rms {rms:.3e} cell")
     for k in ("xi0", "pi0", "dJ_ds0"):
         e, _, _ = _gradient_errors(gold, out, k)
         print(f"configs[2] fp64 transforms {k}: rel L2 {e:.3e}")
