@@ -598,12 +598,22 @@ __global__ void __launch_bounds__(FFT_T) fft_z_r2c_kernel(FftGeom g, float *data
         const int r = threadIdx.x & (ZROWS - 1);
         if (r < nr) {
 #pragma unroll 4
-            for (int k = threadIdx.x >> ZRS; k <= M; k += FFT_T >> ZRS) {
-                const int km = k == M ? 0 : k, kc = (k == 0 || k == M) ? 0 : M - k;
-                const float2 a = tile[ZT(posz[km]) + r], b = tile[ZT(posz[kc]) + r];
-                const float2 E = make_float2(0.5f * (a.x + b.x), 0.5f * (a.y - b.y));
-                const float2 O = make_float2(0.5f * (a.y + b.y), -0.5f * (a.x - b.x));  // (a - conj b) / (2i)
-                outb[k * ZP + r] = cadd(E, cmul(twr[k], O));
+            // one thread per PAIR (k, M - k): X_k = E + w^k O and X_{M-k} = conj(E - w^k O) from one read of Z_k, Z_{M-k}
+            // and one twiddle (half the shared-memory reads of a loop over all k)
+            for (int k = threadIdx.x >> ZRS; k <= M / 2; k += FFT_T >> ZRS) {
+                const float2 a = tile[ZT(posz[k]) + r];
+                if (k == 0) {
+                    outb[r] = make_float2(a.x + a.y, 0.f);               // X_0
+                    outb[M * ZP + r] = make_float2(a.x - a.y, 0.f);      // X_M (Nyquist)
+                } else {
+                    const float2 b = tile[ZT(posz[M - k]) + r];
+                    const float2 E = make_float2(0.5f * (a.x + b.x), 0.5f * (a.y - b.y));
+                    const float2 O = make_float2(0.5f * (a.y + b.y), -0.5f * (a.x - b.x));  // (a - conj b) / (2i)
+                    const float2 t = cmul(twr[k], O);
+                    outb[k * ZP + r] = cadd(E, t);
+                    const float2 d = csub(E, t);
+                    if (2 * k != M) outb[(M - k) * ZP + r] = make_float2(d.x, -d.y);
+                }
             }
         }
     }
@@ -647,11 +657,13 @@ __global__ void __launch_bounds__(FFT_T) fft_z_c2r_kernel(FftGeom g, float *data
         const int r = threadIdx.x & (ZROWS - 1);
         if (r < nr) {
 #pragma unroll 4
-            for (int k = threadIdx.x >> ZRS; k < M; k += FFT_T >> ZRS) {
+            // one thread per PAIR (k, M - k): Z_k = E + i O and Z_{M-k} = conj(E - i O) from one read of X_k, X_{M-k}
+            for (int k = threadIdx.x >> ZRS; k <= M / 2; k += FFT_T >> ZRS) {
                 const float2 a = inb[r * (M + 2) + k], b = inb[r * (M + 2) + M - k];
                 const float2 E = make_float2(a.x + b.x, a.y - b.y);
                 const float2 O = cmulc(make_float2(a.x - b.x, a.y + b.y), twr[k]);
                 tile[ZT(posz[k]) + r] = make_float2(E.x - O.y, E.y + O.x);  // E + i O
+                if (k != 0 && 2 * k != M) tile[ZT(posz[M - k]) + r] = make_float2(E.x + O.y, O.x - E.y);
             }
         }
     }
