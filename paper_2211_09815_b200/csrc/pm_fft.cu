@@ -117,9 +117,15 @@ struct NoOut {
 // OUT = NoOut: the stage works in place on the tile.  Any other OUT receives the results instead -- out(position, column,
 // value) -- so that the LAST stage of a transform can hand them straight to global memory (no store to the tile, no
 // barrier, no copy-out pass).
-template <int N, int L, bool INV, int PITCH, int CS, class OUT>
-__device__ __forceinline__ void fft_stage_impl(float2 *tile, int ncol, const float2 *tw, const OUT &out)
+struct NoIn {
+    __device__ __forceinline__ float2 operator()(int, int) const { return make_float2(0.f, 0.f); }
+};
+// IN = NoIn: the stage reads the tile.  Any other IN supplies the inputs instead -- in(position, column) -- so that the
+// FIRST stage of a transform can take them from where they already are (the z pass: the row-major staging area).
+template <int N, int L, bool INV, int PITCH, int CS, class OUT, class IN = NoIn>
+__device__ __forceinline__ void fft_stage_impl(float2 *tile, int ncol, const float2 *tw, const OUT &out, const IN &in = IN())
 {
+    constexpr bool FROM_TILE = std::is_same<IN, NoIn>::value;
     constexpr int R = stage_radix(L);
     constexpr int Lr = L / R, twstep = N / L;
     constexpr int nwork = (N / R) << CS;
@@ -136,7 +142,8 @@ __device__ __forceinline__ void fft_stage_impl(float2 *tile, int ncol, const flo
         float2 *p = tile + (SAME ? trow<SWZ>(base) : base) * PITCH + col;
         float2 v[R];
 #pragma unroll
-        for (int m = 0; m < R; m++) v[m] = SAME ? p[m * Lr * PITCH] : tile[trow<SWZ>(base + m * Lr) * PITCH + col];
+        for (int m = 0; m < R; m++)
+            v[m] = !FROM_TILE ? in(base + m * Lr, col) : (SAME ? p[m * Lr * PITCH] : tile[trow<SWZ>(base + m * Lr) * PITCH + col]);
         if (INV && Lr > 1) {
 #pragma unroll
             for (int q = 1; q < R; q++) v[q] = cmulc(v[q], tw[j * q * twstep]);
@@ -550,6 +557,13 @@ __global__ void __launch_bounds__(FFT_T, PM_X_MINBLOCKS(NX, CS)) fft_x_adjoint_k
     P::inv_rest(tile, ncol, tw, out_psi);  // the last stage stores psi
 }
 
+// input (position, row) of the z pass from the row-major staging area [row][pitch]
+struct StageIn {
+    const float2 *base;
+    int pitch;
+    __device__ __forceinline__ float2 operator()(int pos, int row) const { return base[row * pitch + pos]; }
+};
+
 // ---- z pass, real -> half-complex, in place on ZROWS consecutive z-rows per CTA ---------------------------------
 // row = [zs floats] -> [zsc complex]; x_n real, n < Nz = 2M: z_n = x_2n + i x_2n+1, Z = FFT_M(z),
 // E_k = (Z_k + conj Z_{M-k}) / 2, O_k = (Z_k - conj Z_{M-k}) / (2i), X_k = E_k + w^k O_k, w = e^{-2 pi i / Nz}, k = 0..M
@@ -584,15 +598,13 @@ __global__ void __launch_bounds__(FFT_T) fft_z_r2c_kernel(FftGeom g, float *data
     }
     fft_cp_async_wait_all();
     __syncthreads();
+    // z_n = x_2n + i x_2n+1 is element n of the staged row: the first stage reads it there (no transposing fill pass)
     {
-        const int r = threadIdx.x & (ZROWS - 1);
-        if (r < nr) {
-#pragma unroll 4
-            for (int n = threadIdx.x >> ZRS; n < M; n += FFT_T >> ZRS) tile[ZT(n) + r] = *reinterpret_cast<const float2 *>(stage + r * (2 * M + 4) + 2 * n);
-        }
+        const StageIn sin = {reinterpret_cast<const float2 *>(stage), M + 2};
+        fft_stage_impl<M, M, false, TP, ZRS, NoOut, StageIn>(tile, nr, tw, NoOut(), sin);
+        __syncthreads();
+        AxisFFTPartial<M, M / stage_radix(M), false, TP, ZRS, 1>::run(tile, nr, tw);
     }
-    __syncthreads();
-    AxisFFT<M, M, false, TP, ZRS>::run(tile, nr, tw);
 
     {
         const int r = threadIdx.x & (ZROWS - 1);
