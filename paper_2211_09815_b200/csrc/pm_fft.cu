@@ -557,6 +557,12 @@ __global__ void __launch_bounds__(FFT_T, PM_X_MINBLOCKS(NX, CS)) fft_x_adjoint_k
     P::inv_rest(tile, ncol, tw, out_psi);  // the last stage stores psi
 }
 
+// result (position, row) of the z pass into the row-major staging area [row][pitch]
+struct StoreOutRow {
+    float2 *base;
+    int pitch;
+    __device__ __forceinline__ void operator()(int pos, int row, float2 v) const { base[row * pitch + pos] = v; }
+};
 // input (position, row) of the z pass from the row-major staging area [row][pitch]
 struct StageIn {
     const float2 *base;
@@ -680,6 +686,21 @@ __global__ void __launch_bounds__(FFT_T) fft_z_c2r_kernel(FftGeom g, float *data
         }
     }
     __syncthreads();
+    if (ZRS == 3) {
+        // 8 unpadded rows: reading the tile along n for the row-wise store would put every lane on two banks.  The last
+        // stage hands its results to the (free again) row-major staging area instead, and the rows leave from there.
+        AxisFFTPartial<M, M / stage_radix(M), true, TP, ZRS, 1>::run(tile, nr, tw);
+        float2 *stage2 = inb;
+        const StoreOutRow so = {stage2, M + 2};
+        fft_stage_impl<M, M, true, TP, ZRS>(tile, nr, tw, so);
+        __syncthreads();
+        float2 *rows2 = reinterpret_cast<float2 *>(rows);
+        for (int idx = threadIdx.x; idx < nr * (M / 2); idx += FFT_T) {
+            const int r = idx / (M / 2), c = idx - r * (M / 2);
+            *reinterpret_cast<float4 *>(rows2 + (size_t)r * (M + 2) + 2 * c) = *reinterpret_cast<const float4 *>(stage2 + r * (M + 2) + 2 * c);
+        }
+        return;
+    }
     AxisFFT<M, M, true, TP, ZRS>::run(tile, nr, tw);
     if (M <= FFT_T) {
         constexpr int RPP = FFT_T / M > 0 ? FFT_T / M : 1;
