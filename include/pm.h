@@ -198,6 +198,21 @@ size_t pm_optimize_ic_scratch_bytes(const pm_ctx *ctx);
 int pm_optimize_ic(pm_ctx *ctx, float *dev_omega, const float *dev_delta_target, double amp, double ns, double rc, int order,
                    int n_iter, double lr, void *dev_scratch, size_t scratch_bytes, double *host_J_history);
 
+/* ---- an entry point that allocates nothing ---------------------------------------------------------------------------
+ * pm_objective's reduction on caller-provided flat arrays, for callers that cannot allocate (CUDA graph capture, serving
+ * loops): r_i = rho_i / nbar - 1 - delta_target_i, *dev_J = 1/2 sum_i r_i^2 (fp64, fixed order: bit-reproducible);
+ * dev_resid[n] receives r when not NULL (may alias dev_rho).  No ctx, no workspace, no cudaMalloc / cudaFree: the per-block
+ * partial sums live in a static device array of 128 KB that every GPU loading the library holds until exit, which limits
+ * n to PM_NOALLOC_MAX_N (a 1024^3 mesh); larger n is PM_EINVAL with the limit in pm_last_error(NULL).  Enqueues two
+ * kernels on cuda_stream and returns without synchronising.  All calls on a device share that array: calls that overlap
+ * on the GPU (different streams, unordered) race on it -- order them.  pm_noalloc_setup resolves the array's device
+ * address for the CURRENT device (the first pm_objective_noalloc on a device does it itself; call it beforehand where the
+ * first call would fall inside a graph capture). */
+#define PM_NOALLOC_MAX_N (1ll << 30)
+int pm_noalloc_setup(void);
+int pm_objective_noalloc(int64_t n, const float *dev_rho, const float *dev_delta_target, double nbar, float *dev_resid,
+                         double *dev_J, void *cuda_stream);
+
 /* ---- instrumentation ---------------------------------------------------------------------------------
  * When enabled, every kernel launch / cuFFT call of the library is bracketed by CUDA events on the
  * ctx's stream.  pm_timing_read SYNCHRONISES, sums the elapsed time per kernel class since the last

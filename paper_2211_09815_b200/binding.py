@@ -60,6 +60,8 @@ _SIGS = {
     "pm_adam_step": (_int, [_vp, _i64, _vp, _vp, _vp, _vp, _int, _dbl, _dbl, _dbl, _dbl]),
     "pm_optimize_ic_scratch_bytes": (C.c_size_t, [_vp]),
     "pm_optimize_ic": (_int, [_vp, _vp, _vp, _dbl, _dbl, _dbl, _int, _int, _dbl, _vp, C.c_size_t, C.POINTER(_dbl)]),
+    "pm_noalloc_setup": (_int, []),
+    "pm_objective_noalloc": (_int, [_i64, _vp, _vp, _dbl, _vp, _vp, _vp]),
     "pm_scatter": (_int, [_vp, _i64, _vp, _vp, _int, _vp]),
     "pm_gather": (_int, [_vp, _i64, _vp, _vp, _int, _vp]),
     "pm_gather_grad": (_int, [_vp, _i64, _vp, _vp, _int, _vp, _vp]),
@@ -133,6 +135,19 @@ def host_ic_factors(omega_m, a0):
     if rc != PM_OK:
         raise PMError(rc, "pm_host_ic_factors")
     return list(out)
+
+
+PM_NOALLOC_MAX_N = 1 << 30
+
+
+def objective_noalloc(rho, delta_target, nbar, J, resid=None, stream=None):
+    """pm_objective_noalloc: J[0] (float64 CUDA tensor of the caller) = 1/2 sum (rho / nbar - 1 - delta_target)^2 over the
+    flat arrays; libpm allocates nothing for it (static device scratch, n <= PM_NOALLOC_MAX_N).  Asynchronous."""
+    st = stream if stream is not None else torch.cuda.current_stream(rho.device)
+    rc = _lib.pm_objective_noalloc(rho.numel(), _ptr(rho, "rho"), _ptr(delta_target, "delta_target"), float(nbar),
+                                   _ptr(resid, "resid"), _ptr(J, "J", torch.float64), st.cuda_stream)
+    if rc != PM_OK:
+        raise PMError(rc, _lib.pm_last_error(None).decode())
 
 
 def host_fft_order(n):
