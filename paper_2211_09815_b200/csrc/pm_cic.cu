@@ -72,6 +72,7 @@ constexpr int NCW = 8;                                    // consumer warps
 constexpr int NCT = NCW * 32;                             // consumer threads
 constexpr int NTHREADS = NCT + 32;                        // + one producer warp
 constexpr int SCHUNK = 2048;                               // scatter: records per chunk of a heavy tile
+constexpr int SFAST = 1024;                               // valued scatter: tiles up to this many records take their bound from an integer sum
 constexpr int RCAP = 512;                                 // records staged in shared memory per tile (the rest are read from global)
 
 // ---- PTX wrappers: mbarrier + TMA (sm_90+/sm_100a) ----------------------------------------------------
@@ -485,6 +486,7 @@ __global__ void __launch_bounds__(NTHREADS) scatter_kernel(const __grid_constant
     __shared__ __align__(8) unsigned long long full[NST], empty[NST];
     __shared__ ScatterSlot slot[NST];
     __shared__ float redf[NCW];
+    __shared__ unsigned redu[NCW];
     __shared__ int heavy_last;
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -736,6 +738,33 @@ __global__ void __launch_bounds__(NTHREADS) scatter_kernel(const __grid_constant
             vmax = consumer_max(vmax, redf);
             scale = 1.f;
             if (total > 0 && vmax > 0.f && vmax < 3e38f) {
+              float bound;
+              if (total <= SFAST) {
+                // Light tile (the normal case: 256 records on average): no point's sum can exceed sum_i max_c |v_i,c| (weights
+                // are <= 1).  That sum is formed in INTEGER units of vmax 2^-20, each term rounded up, so it does not depend on
+                // the order of the records either, and it replaces the bound pass below (8 atomics per record, a scan of the
+                // tile, two barriers).  For heavy tiles it would be far too loose at the sparse points of the tile.
+                const float inv = 1048576.f / vmax;
+                unsigned qs = 0u;
+                if (ia < total) qs += (unsigned)(ma * inv) + 2u;
+                if (ib < total) qs += (unsigned)(mb * inv) + 2u;
+                for (int i = ib + NCT; i < total; i += NCT) {
+                    float v[C], m = 0.f;
+                    values(fetch(i), v);
+#pragma unroll
+                    for (int c = 0; c < C; c++) m = fmaxf(m, fabsf(v[c]));
+                    qs += (unsigned)(m * inv) + 2u;
+                }
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) qs += __shfl_xor_sync(0xffffffffu, qs, o);
+                if (lane == 0) redu[warp] = qs;
+                consumer_sync();
+                qs = 0u;
+#pragma unroll
+                for (int k2 = 0; k2 < NCW; k2++) qs += redu[k2];
+                consumer_sync();
+                bound = ((float)qs * 1.0000002f) * (vmax * (1.f / 1048576.f)) * 1.001f;
+              } else {
                 const float sA = __uint_as_float((unsigned)(127 + min(31 - exp_above(fmaxf((float)total * vmax, 1e-30f)), 96)) << 23);
                 auto pass_a = [&](int i, uint4 q, float m) {
                     const float ms = m * sA;
@@ -764,7 +793,8 @@ __global__ void __launch_bounds__(NTHREADS) scatter_kernel(const __grid_constant
                     tile_acc[i] = 0;
                 }
                 const float M = consumer_max((float)um * 1.0000002f, redf);  // (float) may round down: one ulp up
-                const float bound = (M + 0.5f * (float)total + 1.f) / sA * 1.001f;
+                bound = (M + 0.5f * (float)total + 1.f) / sA * 1.001f;
+              }
                 const int k = min(30 - exp_above(fmaxf(bound, 1e-37f)), 96) - PM_DBG(g.kshift);
                 scale = __uint_as_float((unsigned)(127 + k) << 23);
                 auto pass_b = [&](int i, uint4 q, const float v[C]) {
