@@ -326,6 +326,36 @@ def run_ours(args):
         pm.timing_enable(False)
         pm.timing_reset()
 
+    # forward-only and adjoint-only rates through the step-by-step ABI calls (pm_set_state + n pm_step_fwd;
+    # pm_objective + n pm_step_adj): the same kernels as the whole run without the chaining of kick / drift across steps
+    split = None
+    if world == 1 and not args.no_kernel_timing:
+        def fwd_only():
+            pm.set_state(s0d, p0d)
+            for i in range(1, n + 1):
+                pm.step_fwd(i)
+
+        def adj_only():
+            pm.objective(tgd)
+            for i in range(n, 0, -1):
+                pm.step_adj(i)
+
+        fwd_only()
+        adj_only()
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+        torch.cuda.synchronize()
+        ev[0].record(stream)
+        fwd_only()
+        ev[1].record(stream)
+        adj_only()
+        ev[2].record(stream)
+        torch.cuda.synchronize()
+        tf, ta = ev[0].elapsed_time(ev[1]), ev[1].elapsed_time(ev[2])
+        split = {"forward_only": {"value": npart * n / (tf * 1e-3), "unit": UNIT, "ms": tf},
+                 "adjoint_only": {"value": npart * n / (ta * 1e-3), "unit": UNIT, "ms": ta},
+                 "note": "step-by-step ABI calls (acc_0 billed to the forward part, the objective to the adjoint part), "
+                         "1 warm-up + 1 timed pass; the whole run chains kick / drift across steps and is faster than the sum"}
+
     # end to end through host buffers (e2e): H2D of inputs and D2H of results inside the timed region
     hin = [torch.from_numpy(v).pin_memory() for v in (s0, p0, target)]
     hout = {k: torch.empty((npart, 3), dtype=torch.float32).pin_memory() for k in ("s_n", "p_n", "dJ_ds0")}
@@ -361,6 +391,8 @@ def run_ours(args):
                 "ms_per_step_instrumented": None if ms_instr is None else ms_instr / args.steps,
                 "clocks": clk, "roofline": graded_roofline(kernels, cfg["name"], peak, peak_src), "kernels": kernels,
                 "objective_J": J[0], "peak_mem_GB": peak_mem, "workspace_GB": ws_gb}
+        if split:
+            line["split"] = split
         if world == 1 and not args.no_cpu_baseline:
             n_pairs = args.cpu_pairs
             v, tf, ta, threads = oracle_steady_sample(cfg, s0, p0, target, n_pairs)
