@@ -14,6 +14,9 @@ section 9 has the arithmetic).  The same JSON line carries, at N = 1:
                   peak-memory triple for n = 25, 50, 100 steps (torch peak + cudaMemGetInfo delta);
   sweep.cfg4      configs[4]: CIC scatter / gather / weight-gradient gather of 512^3 particles on a 1024^3 mesh,
                   clustered vs uniform positions, generation vs random memory order, kernel-only and with binning.
+  split           forward-only and adjoint-only rates of the headline workload (step-by-step ABI calls);
+  modes           the headline workload in the fp64-transform mode (pm_params.flags, the mode that meets the 1e-3 gradient bar);
+  next_rows       milliseconds per call of the SURVEY 8f rows (device ICs and their VJP, observed snapshots, dJ/dOmega_m, Adam).
 N > 1 (torchrun): the path does not shard; every rank runs an independent
 replica on its own seed, no collective in the data path, value = sum over ranks / max time.
 --impl reference times the CPU fp64 ORACLE (oracle/) on bounded samples of the same workload.
